@@ -1,0 +1,143 @@
+/*
+ * obem.h -- C ABI of libobem.so: the B200-native (sm_100a) field-evaluation hot path of the
+ * OuroborosBEM method (arXiv 2110.09214).
+ *
+ * What the library computes, for every target point r (a tracked charge, or an arbitrary point):
+ *
+ *   N-body part   PAPER.md:272-277, section 3.2.4, Eq (3.8):
+ *       E_Nbody(r_p') = 1/(4 pi eps0) * sum_{p != p'} q_p (r_p' - r_p) / ||r_p' - r_p||^3
+ *     with Plummer softening (reading A2): r2 = ||d||^2 + eps_pp^2, E += q d r2^(-3/2),
+ *     phi += q r2^(-1/2).  At the charges the self term p = p' is excluded BY INDEX (reading A3).
+ *
+ *   Panel part    PAPER.md:141-147, section 2.2, Eq (2.13), (2.14):
+ *       V(r) = sum_i sigma_i/(4 pi eps0) Int_{C_i} 1/||r-r'|| d2r'
+ *       E(r) = sum_i sigma_i/(4 pi eps0) Int_{C_i} (r-r')/||r-r'||^3 d2r'
+ *     sigma_i constant over the flat triangular cell C_i; the cell integral is the
+ *     7-point degree-5 triangle rule (reading A1).
+ *
+ *   The two parts are superposed.  A source at exactly zero (softened) distance
+ *   contributes 0 (reading A4).
+ *
+ * Conventions
+ *   - SI units: metres, coulombs, C/m^2, V/m, V.   k_e = 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m.
+ *   - All arithmetic on the device is fp32 (two-level fp32 accumulation, fp64 only in the O(N) pack
+ *     and fix-up steps).  Every step of the path runs in the library's CUDA kernels.
+ *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors), 16-byte
+ *     aligned; pointers named h_* are HOST pointers.  The library copies / repacks on set_* into
+ *     buffers it owns: an input may be freed or overwritten as soon as the stream has passed the
+ *     call.  Outputs are caller-owned and fully overwritten.
+ *   - All device work is enqueued on the caller's stream (`cuda_stream` is a cudaStream_t passed as
+ *     void*; NULL = the legacy default stream).  No hidden synchronisation and no host copies,
+ *     except: (a) a set_* / eval_* call that must GROW a library-owned buffer calls cudaMalloc,
+ *     which may synchronise the device (obem_reserve avoids it); (b) the *_host entry points,
+ *     which are synchronous by contract.
+ *   - Every entry point returns an obem_status (0 = OK, negative = error); nothing throws across
+ *     the ABI.  n = 0 / n_panels = 0 / m = 0 are valid.  There is no CPU fallback: without a
+ *     CUDA device obem_create fails with OBEM_ECUDA.
+ *   - A context is bound to one device and is not thread-safe; use one context per thread/stream.
+ */
+#ifndef OBEM_H
+#define OBEM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct obem_ctx obem_ctx; /* opaque; one per device (per stream of use) */
+
+typedef enum obem_status {
+    OBEM_OK = 0,
+    OBEM_EINVAL = -1, /* null / negative / misaligned argument, unknown flag bits            */
+    OBEM_ESTATE = -2, /* evaluate before the sources the flags ask for were set              */
+    OBEM_ECUDA = -3,  /* a CUDA call failed; obem_last_cuda_error() gives the cudaError_t     */
+    OBEM_ENOMEM = -4  /* device allocation failed                                            */
+} obem_status;
+
+/* flags of the evaluate calls: which of the two sums to include */
+#define OBEM_NBODY 1u  /* Eq (3.8), sources = the charges of obem_set_charges              */
+#define OBEM_PANELS 2u /* Eq (2.13)/(2.14), sources = the panels of obem_set_panels         */
+
+/* Create a context on CUDA device `device`.  Queries the SM count and sizes the persistent grid.
+ * *out is NULL on failure. */
+int obem_create(obem_ctx** out, int device);
+
+/* Free the context and every library-owned device buffer.  Synchronises the device.  NULL is OK. */
+int obem_destroy(obem_ctx* c);
+
+/* Pre-allocate library-owned buffers for up to n_charges charges and n_panels panels, so that later
+ * set_* calls never allocate (and therefore never synchronise).  Optional. */
+int obem_reserve(obem_ctx* c, int64_t n_charges, int64_t n_panels);
+
+/* Softening lengths in metres, >= 0 and finite.  eps_pp: charge-charge sum (reading A2; 0 = Eq 3.8
+ * as printed).  eps_panel: panel sum (reading A5; default 0).  Defaults 0, 0.  Takes effect at the
+ * next evaluate call. */
+int obem_set_softening(obem_ctx* c, float eps_pp_m, float eps_panel_m);
+
+/* Panels (flat cells with constant sigma; triangles only, reading A8).
+ *   d_verts [n_panels][3][3] fp32: vertex j of panel p at d_verts[(p*3+j)*3 + 0..2] = x,y,z [m]
+ *   d_sigma [n_panels] fp32 [C/m^2]
+ * Derives, in fp64 and rounded once to fp32, the area A_p and the 7 quadrature sources
+ * (x_pk, sigma_p*A_p*w_k) of every panel.  Replaces any earlier panel set.  Degenerate (A = 0)
+ * panels contribute 0. */
+int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int64_t n_panels,
+                    void* cuda_stream);
+
+/* New sigma on the SAME geometry (charging-up changes sigma every step, Eq 3.7):
+ * rescales the weights only.  n_panels must equal the count of the last obem_set_panels
+ * (else OBEM_EINVAL; OBEM_ESTATE if no panels were ever set). */
+int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cuda_stream);
+
+/* Charges (Eq 3.8's particles): d_xyzq [n][4] fp32 = x, y, z [m], q [C].  Replaces any earlier set. */
+int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_stream);
+
+/* E and phi at the charges themselves: d_out [n][4] fp32 = Ex, Ey, Ez [V/m], phi [V].
+ * With OBEM_NBODY the sum over charges excludes the target's own index.  A flag whose sources are
+ * an EMPTY set contributes 0; a flag whose sources were NEVER set gives OBEM_ESTATE. */
+int obem_eval_at_charges(obem_ctx* c, float* d_out, unsigned flags, void* cuda_stream);
+
+/* Same, for the contiguous slice [first, first+count) of the charges only: d_out [count][4].
+ * This is the multi-GPU sharding unit (targets sharded across ranks, sources replicated). */
+int obem_eval_at_charges_range(obem_ctx* c, int64_t first, int64_t count, float* d_out,
+                               unsigned flags, void* cuda_stream);
+
+/* E and phi at arbitrary points (field map / static option):
+ *   d_pts [m][4] fp32, 4th lane ignored;  d_out [m][4].
+ * With OBEM_NBODY all charges are summed with the same softening and NO exclusion. */
+int obem_eval_at_points(obem_ctx* c, const float* d_pts, int64_t m, float* d_out, unsigned flags,
+                        void* cuda_stream);
+
+/* The whole hot path through HOST buffers, synchronous: copies the inputs to the device, runs
+ * set_panels (if h_verts != NULL; if NULL the panels already set are kept), set_charges, the
+ * evaluation at the charges, and copies the result back.  Pageable or pinned host memory. */
+int obem_field_at_charges_host(obem_ctx* c, const float* h_xyzq, int64_t n, const float* h_verts,
+                               const float* h_sigma, int64_t n_panels, float* h_out, unsigned flags);
+
+/* Field map through HOST buffers, synchronous (h_verts may be NULL as above). */
+int obem_field_at_points_host(obem_ctx* c, const float* h_pts, int64_t m, const float* h_verts,
+                              const float* h_sigma, int64_t n_panels, float* h_out, unsigned flags);
+
+/* Introspection (host side, no device work) */
+int64_t obem_n_charges(const obem_ctx* c);     /* -1 if never set */
+int64_t obem_n_panels(const obem_ctx* c);      /* -1 if never set */
+int obem_sm_count(const obem_ctx* c);          /* multiprocessors of the device                     */
+int obem_grid_size(const obem_ctx* c);         /* CTAs of the persistent evaluation kernel          */
+int64_t obem_kernel_launches(const obem_ctx* c); /* kernels this context has launched so far          */
+int obem_last_cuda_error(const obem_ctx* c);   /* cudaError_t of the last failed CUDA call, else 0   */
+const char* obem_status_string(int status);
+
+/* Copy the packed quadrature sources (x, y, z, sigma*A*w_k) of the current panel set to
+ * d_out [n_panels*7][4] fp32 -- for inspection and tests. */
+int obem_get_panel_sources(obem_ctx* c, float* d_out, void* cuda_stream);
+
+/* FP32 pipe microbenchmark (measurement aid for the roofline denominator, not on the hot path):
+ * launches a register-only chain of `iters` dependent-free FFMA (mode 0) or packed FFMA2 (mode 1)
+ * instructions per thread on the persistent grid and returns the flop count it executed in
+ * *flops_out (2 per scalar FMA).  Time it with events on `cuda_stream`. */
+int obem_fma_peak_probe(obem_ctx* c, int mode, int64_t iters, double* flops_out, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OBEM_H */

@@ -1,0 +1,301 @@
+"""Thin ctypes binding of libobem.so (include/obem.h).  Argument marshalling only: every step of the
+path runs in the library's CUDA kernels.  torch is used for device memory and streams.
+
+There is NO CPU fallback: if libobem.so is missing or does not load, importing this module raises;
+if there is no CUDA device, `Context()` raises (obem_create -> OBEM_ECUDA).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+NBODY = 1   # OBEM_NBODY  -- Eq (3.8)
+PANELS = 2  # OBEM_PANELS -- Eq (2.13)/(2.14)
+
+_c_fp = ctypes.c_void_p  # device or host float* passed as an address
+_i64 = ctypes.c_int64
+
+# every symbol include/obem.h declares: name -> (restype, argtypes)
+SIGNATURES = {
+    "obem_create": (ctypes.c_int, [ctypes.POINTER(ctypes.c_void_p), ctypes.c_int]),
+    "obem_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "obem_reserve": (ctypes.c_int, [ctypes.c_void_p, _i64, _i64]),
+    "obem_set_softening": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float, ctypes.c_float]),
+    "obem_set_panels": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_void_p]),
+    "obem_set_sigma": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, ctypes.c_void_p]),
+    "obem_set_charges": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, ctypes.c_void_p]),
+    "obem_eval_at_charges": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_uint, ctypes.c_void_p]),
+    "obem_eval_at_charges_range": (ctypes.c_int, [ctypes.c_void_p, _i64, _i64, _c_fp, ctypes.c_uint,
+                                                  ctypes.c_void_p]),
+    "obem_eval_at_points": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, _c_fp, ctypes.c_uint, ctypes.c_void_p]),
+    "obem_field_at_charges_host": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, _c_fp, _c_fp, _i64, _c_fp,
+                                                  ctypes.c_uint]),
+    "obem_field_at_points_host": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, _c_fp, _c_fp, _i64, _c_fp,
+                                                 ctypes.c_uint]),
+    "obem_n_charges": (_i64, [ctypes.c_void_p]),
+    "obem_n_panels": (_i64, [ctypes.c_void_p]),
+    "obem_sm_count": (ctypes.c_int, [ctypes.c_void_p]),
+    "obem_grid_size": (ctypes.c_int, [ctypes.c_void_p]),
+    "obem_kernel_launches": (_i64, [ctypes.c_void_p]),
+    "obem_last_cuda_error": (ctypes.c_int, [ctypes.c_void_p]),
+    "obem_status_string": (ctypes.c_char_p, [ctypes.c_int]),
+    "obem_get_panel_sources": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
+    "obem_fma_peak_probe": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, _i64, ctypes.POINTER(ctypes.c_double),
+                                           ctypes.c_void_p]),
+}
+
+LIB_PATH = _build.LIB
+
+
+def load_library(path: str = LIB_PATH) -> ctypes.CDLL:
+    """dlopen libobem.so and bind every declared symbol; raises if the library or a symbol is missing."""
+    if not os.path.exists(path):
+        raise ImportError(
+            "libobem.so not found at %s: build it with `python -m paper_2110_09214_b200.build` "
+            "(__graft_entry__.build()).  There is no CPU fallback." % path)
+    lib = ctypes.CDLL(path)
+    for name, (res, args) in SIGNATURES.items():
+        fn = getattr(lib, name)  # AttributeError if the symbol is not exported
+        fn.restype = res
+        fn.argtypes = args
+    return lib
+
+
+_lib = load_library()
+
+
+class ObemError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda_error: int = 0):
+        self.status = status
+        self.cuda_error = cuda_error
+        msg = _lib.obem_status_string(status).decode()
+        if cuda_error:
+            msg += " [cudaError_t %d]" % cuda_error
+        super().__init__("%s: %s" % (where, msg))
+
+
+def status_string(status: int) -> str:
+    return _lib.obem_status_string(int(status)).decode()
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dev_f32(t, what, last=None):
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous float32 CUDA tensor" % what)
+    if last is not None and (t.dim() < 1 or tuple(t.shape[-len(last):]) != tuple(last)):
+        raise ValueError("%s must have trailing shape %r, got %r" % (what, last, tuple(t.shape)))
+    return t
+
+
+def _stream_ptr(stream):
+    torch = _torch()
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+class Context:
+    """One obem_ctx on one CUDA device.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, device: int = 0):
+        self._h = ctypes.c_void_p()
+        self.device = int(device)
+        rc = _lib.obem_create(ctypes.byref(self._h), self.device)
+        if rc != 0:
+            self._h = ctypes.c_void_p()
+            raise ObemError(rc, "obem_create(device=%d)" % device)
+
+    # -- lifetime ---------------------------------------------------------------------------------
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            _lib.obem_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    close = destroy
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def _check(self, rc, where):
+        if rc != 0:
+            raise ObemError(rc, where, _lib.obem_last_cuda_error(self._h))
+
+    # -- setters ----------------------------------------------------------------------------------
+    def reserve(self, n_charges: int, n_panels: int):
+        self._check(_lib.obem_reserve(self._h, int(n_charges), int(n_panels)), "obem_reserve")
+
+    def set_softening(self, eps_pp: float, eps_panel: float = 0.0):
+        self._check(_lib.obem_set_softening(self._h, float(eps_pp), float(eps_panel)), "obem_set_softening")
+
+    def set_panels(self, verts, sigma, stream=None):
+        """verts [Np,3,3], sigma [Np] float32 CUDA tensors."""
+        n = int(sigma.shape[0])
+        if n:
+            _dev_f32(verts, "verts", (3, 3))
+            _dev_f32(sigma, "sigma")
+            if verts.shape[0] != n:
+                raise ValueError("verts and sigma disagree on the number of panels")
+        self._check(_lib.obem_set_panels(self._h, verts.data_ptr() if n else None, sigma.data_ptr() if n else None,
+                                         n, _stream_ptr(stream)), "obem_set_panels")
+
+    def set_sigma(self, sigma, stream=None):
+        n = int(sigma.shape[0])
+        if n:
+            _dev_f32(sigma, "sigma")
+        self._check(_lib.obem_set_sigma(self._h, sigma.data_ptr() if n else None, n, _stream_ptr(stream)),
+                    "obem_set_sigma")
+
+    def set_charges(self, xyzq, stream=None):
+        """xyzq [N,4] float32 CUDA tensor (x, y, z [m], q [C]) -- Eq (3.8)'s particles."""
+        n = int(xyzq.shape[0])
+        if n:
+            _dev_f32(xyzq, "xyzq", (4,))
+        self._check(_lib.obem_set_charges(self._h, xyzq.data_ptr() if n else None, n, _stream_ptr(stream)),
+                    "obem_set_charges")
+
+    # -- evaluation -------------------------------------------------------------------------------
+    def eval_at_charges(self, out=None, flags: int = NBODY | PANELS, stream=None):
+        torch = _torch()
+        n = self.n_charges
+        if n < 0:
+            self._check(-2, "obem_eval_at_charges")
+        if out is None:
+            out = torch.empty((n, 4), dtype=torch.float32, device="cuda:%d" % self.device)
+        elif n:
+            _dev_f32(out, "out", (4,))
+            if out.shape[0] != n:
+                raise ValueError("out must be [n_charges, 4]")
+        self._check(_lib.obem_eval_at_charges(self._h, out.data_ptr() if n else None, int(flags), _stream_ptr(stream)),
+                    "obem_eval_at_charges")
+        return out
+
+    def eval_at_charges_range(self, first: int, count: int, out=None, flags: int = NBODY | PANELS, stream=None):
+        torch = _torch()
+        if out is None:
+            out = torch.empty((max(count, 0), 4), dtype=torch.float32, device="cuda:%d" % self.device)
+        elif count > 0:
+            _dev_f32(out, "out", (4,))
+            if out.shape[0] != count:
+                raise ValueError("out must be [count, 4]")
+        self._check(_lib.obem_eval_at_charges_range(self._h, int(first), int(count),
+                                                    out.data_ptr() if count > 0 else None, int(flags),
+                                                    _stream_ptr(stream)), "obem_eval_at_charges_range")
+        return out
+
+    def eval_at_points(self, pts, out=None, flags: int = PANELS, stream=None):
+        torch = _torch()
+        m = int(pts.shape[0])
+        if m:
+            _dev_f32(pts, "pts", (4,))
+        if out is None:
+            out = torch.empty((m, 4), dtype=torch.float32, device="cuda:%d" % self.device)
+        elif m:
+            _dev_f32(out, "out", (4,))
+            if out.shape[0] != m:
+                raise ValueError("out must be [m, 4]")
+        self._check(_lib.obem_eval_at_points(self._h, pts.data_ptr() if m else None, m,
+                                             out.data_ptr() if m else None, int(flags), _stream_ptr(stream)),
+                    "obem_eval_at_points")
+        return out
+
+    # -- host-buffer entry points (synchronous) ------------------------------------------------------
+    @staticmethod
+    def _host_ptr(a, what, shape_tail):
+        import numpy as np
+        if a is None:
+            return None, 0
+        if not isinstance(a, np.ndarray) or a.dtype != np.float32 or not a.flags["C_CONTIGUOUS"]:
+            raise TypeError("%s must be a C-contiguous float32 numpy array" % what)
+        if a.size and tuple(a.shape[1:]) != tuple(shape_tail):
+            raise ValueError("%s must have shape [n%s]" % (what, "".join(",%d" % s for s in shape_tail)))
+        return (a.ctypes.data if a.size else None), int(a.shape[0])
+
+    def field_at_charges_host(self, xyzq, verts=None, sigma=None, out=None, flags: int = NBODY | PANELS):
+        """Whole path through host (numpy) buffers: H2D, set_panels (if verts given), set_charges,
+        eval_at_charges, D2H.  Returns out [N,4] float32 numpy."""
+        import numpy as np
+        px, n = self._host_ptr(xyzq, "xyzq", (4,))
+        pv, npan = self._host_ptr(verts, "verts", (3, 3))
+        ps, ns = self._host_ptr(sigma, "sigma", ())
+        if verts is not None and ns != npan:
+            raise ValueError("verts and sigma disagree on the number of panels")
+        if out is None:
+            out = np.empty((n, 4), dtype=np.float32)
+        po, no = self._host_ptr(out, "out", (4,))
+        if no != n:
+            raise ValueError("out must be [n, 4]")
+        if verts is not None and npan == 0:
+            pv = ctypes.addressof(ctypes.c_float())  # non-NULL marker: "set an empty panel set"
+        self._check(_lib.obem_field_at_charges_host(self._h, px, n, pv, ps, npan, po, int(flags)),
+                    "obem_field_at_charges_host")
+        return out
+
+    def field_at_points_host(self, pts, verts=None, sigma=None, out=None, flags: int = PANELS):
+        import numpy as np
+        pp, m = self._host_ptr(pts, "pts", (4,))
+        pv, npan = self._host_ptr(verts, "verts", (3, 3))
+        ps, ns = self._host_ptr(sigma, "sigma", ())
+        if verts is not None and ns != npan:
+            raise ValueError("verts and sigma disagree on the number of panels")
+        if out is None:
+            out = np.empty((m, 4), dtype=np.float32)
+        po, mo = self._host_ptr(out, "out", (4,))
+        if mo != m:
+            raise ValueError("out must be [m, 4]")
+        if verts is not None and npan == 0:
+            pv = ctypes.addressof(ctypes.c_float())
+        self._check(_lib.obem_field_at_points_host(self._h, pp, m, pv, ps, npan, po, int(flags)),
+                    "obem_field_at_points_host")
+        return out
+
+    # -- introspection ----------------------------------------------------------------------------
+    @property
+    def n_charges(self) -> int:
+        return int(_lib.obem_n_charges(self._h))
+
+    @property
+    def n_panels(self) -> int:
+        return int(_lib.obem_n_panels(self._h))
+
+    @property
+    def sm_count(self) -> int:
+        return int(_lib.obem_sm_count(self._h))
+
+    @property
+    def grid_size(self) -> int:
+        return int(_lib.obem_grid_size(self._h))
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(_lib.obem_kernel_launches(self._h))
+
+    def get_panel_sources(self, stream=None):
+        torch = _torch()
+        n = max(self.n_panels, 0)
+        out = torch.empty((n * 7, 4), dtype=torch.float32, device="cuda:%d" % self.device)
+        self._check(_lib.obem_get_panel_sources(self._h, out.data_ptr() if n else None, _stream_ptr(stream)),
+                    "obem_get_panel_sources")
+        return out
+
+    def fma_peak_probe(self, mode: int, iters: int, stream=None) -> float:
+        """Enqueue the FP32-pipe probe; returns the flop count it executes (time it with events)."""
+        fl = ctypes.c_double(0.0)
+        self._check(_lib.obem_fma_peak_probe(self._h, int(mode), int(iters), ctypes.byref(fl), _stream_ptr(stream)),
+                    "obem_fma_peak_probe")
+        return fl.value

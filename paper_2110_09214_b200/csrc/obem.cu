@@ -1,0 +1,902 @@
+/*
+ * obem.cu -- libobem.so: CUDA kernels (sm_100a) and C ABI (include/obem.h) of the OuroborosBEM
+ * field-evaluation hot path (arXiv 2110.09214): Eq (3.8) N-body sum and the
+ * panel sums Eq (2.13)/(2.14) at charges or arbitrary points.
+ *
+ * Design (DESIGN.md has the long form):
+ *   - Both sums are "point source -> target" sums with the same body; a panel is 7 point sources
+ *     (7-point degree-5 rule, reading A1) derived once per geometry in fp64 (pack_panels_kernel).
+ *   - One persistent kernel (obem_eval_kernel) covers charges AND panel sources in one launch.
+ *     Work is the linearised space (target tile, source block); every CTA gets an equal contiguous
+ *     share of it ("stream-K" split), so there is no wave-quantisation tail at any problem size.
+ *     Tiles a CTA covers completely are written directly; tiles split between CTAs go through a
+ *     small fixed-size workspace and a deterministic fix-up kernel (fp64 sum of the partials).
+ *   - Inner loop: 8 targets per thread held as 4 packed f32x2 register pairs; each source is one
+ *     broadcast LDS.128 from a shared-memory ring that a single thread fills with 1-D TMA bulk
+ *     copies (cp.async.bulk + mbarrier); arithmetic is Blackwell's packed FADD2/FMUL2/FFMA2
+ *     (13 per target pair and source) + 2 MUFU.RSQ -- half the issue slots of scalar code at the
+ *     same FP32 lane throughput.
+ *   - fp32 accumulation is two-level: per 256-source block, then flushed into a running sum.
+ *   - No tensor cores: the path is not a dense contraction.  No CPU fallback anywhere.
+ *
+ * This file shares no code, header, table or constant with oracle/.
+ */
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <math.h>
+#include <new>
+
+#include "obem.h"
+
+namespace {
+
+typedef unsigned long long u64;
+
+constexpr int THREADS = 256;          /* threads per CTA of the evaluation kernel                 */
+constexpr int TPT = 8;                /* targets per thread                                        */
+constexpr int NPAIR = TPT / 2;        /* packed f32x2 target pairs per thread                      */
+constexpr int TT = THREADS * TPT;     /* targets per tile (2048)                                   */
+constexpr int SB = 256;               /* sources per shared-memory block (4 KiB)                   */
+constexpr int STAGES = 4;             /* depth of the TMA ring                                     */
+constexpr int CTAS_PER_SM = 2;
+
+/* k_e = 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), reading A7 */
+constexpr double KE_D = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12);
+
+/* ------------------------------------------------------------------------------------------- */
+/* packed f32x2 helpers (PTX ISA: add/sub/mul/fma .f32x2, sm_100+).  A u64 holds {lo, hi}.       */
+/* ------------------------------------------------------------------------------------------- */
+__device__ __forceinline__ u64 pk(float lo, float hi)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk(u64 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
+{
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ u64 add2(u64 a, u64 b)
+{
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 sub2(u64 a, u64 b)
+{
+    u64 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b)
+{
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); /* one MUFU.RSQ */
+    return r;
+}
+
+/* ------------------------------------------------------------------------------------------- */
+/* mbarrier + 1-D TMA bulk copy (global -> shared)                                              */
+/* ------------------------------------------------------------------------------------------- */
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(u64* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, u64* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+/* ------------------------------------------------------------------------------------------- */
+/* evaluation kernel                                                                            */
+/* ------------------------------------------------------------------------------------------- */
+struct Section {
+    const float4* src; /* packed sources (x, y, z, weight), padded to a multiple of SB with weight 0 */
+    long long nblk;    /* number of SB-blocks                                                        */
+    float eps2;        /* softening^2 of this section                                                */
+};
+
+struct EvalParams {
+    Section sec[2];
+    long long nblk;   /* sec[0].nblk + sec[1].nblk                                   */
+    const float4* tgt;
+    long long nt;     /* targets                                                     */
+    long long ntiles; /* ceil(nt / TT)                                               */
+    long long U;      /* work units = ntiles * nblk                                  */
+    float4* out;      /* [nt]                                                        */
+    float4* ws;       /* [grid][2][TT] partial sums of split tiles                   */
+    int self_sub;     /* 1: subtract the target's own softened phi term (reading A3) */
+    float self_eps2;
+};
+
+/* first work unit of CTA c: floor(c * U / G) */
+__device__ __forceinline__ long long unit_begin(long long c, long long U, long long G)
+{
+    return (long long)(((u64)c * (u64)U) / (u64)G);
+}
+
+/*
+ * One shared-memory block of SB sources against the thread's 8 targets.
+ * Per source and target pair: 3 FADD2 (d = r_t - r_s), 3 FFMA2 (r2 = d.d + eps^2), 2 MUFU.RSQ,
+ * FMUL2 (t = w u), FADD2 (phi += t), FMUL2 (u^2), FMUL2 (s = t u^2), 3 FFMA2 (E += s d).
+ * GUARD (eps = 0 only): a source at zero distance contributes 0 (reading A4).
+ */
+template <bool GUARD>
+__device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
+                                           const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
+                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
+{
+    const u64 e2 = pk(eps2, eps2);
+#pragma unroll 2
+    for (int j = 0; j < SB; ++j) {
+        const float4 q = s[j]; /* warp-uniform address: one broadcast LDS.128 */
+        const u64 sx = pk(q.x, q.x), sy = pk(q.y, q.y), sz = pk(q.z, q.z), sw = pk(q.w, q.w);
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) {
+            const u64 dx = sub2(X[p], sx);
+            const u64 dy = sub2(Y[p], sy);
+            const u64 dz = sub2(Z[p], sz);
+            u64 r2 = fma2(dx, dx, e2);
+            r2 = fma2(dy, dy, r2);
+            r2 = fma2(dz, dz, r2);
+            float r2l, r2h;
+            upk(r2, r2l, r2h);
+            float ul = rsqrt_approx(r2l);
+            float uh = rsqrt_approx(r2h);
+            if (GUARD) {
+                ul = (r2l > 0.0f) ? ul : 0.0f;
+                uh = (r2h > 0.0f) ? uh : 0.0f;
+            }
+            const u64 u = pk(ul, uh);
+            const u64 t = mul2(u, sw);
+            aP[p] = add2(aP[p], t);
+            const u64 u2 = mul2(u, u);
+            const u64 sE = mul2(t, u2);
+            aX[p] = fma2(sE, dx, aX[p]);
+            aY[p] = fma2(sE, dy, aY[p]);
+            aZ[p] = fma2(sE, dz, aZ[p]);
+        }
+    }
+}
+
+__device__ __forceinline__ const float4* unit_src(const EvalParams& P, long long blk)
+{
+    return (blk < P.sec[0].nblk) ? P.sec[0].src + blk * SB : P.sec[1].src + (blk - P.sec[0].nblk) * SB;
+}
+
+__global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
+{
+    __shared__ __align__(128) float4 ring[STAGES][SB];
+    __shared__ __align__(8) u64 full[STAGES];
+
+    const int tid = threadIdx.x;
+    const long long G = gridDim.x, c = blockIdx.x;
+    const long long u0 = unit_begin(c, P.U, G), u1 = unit_begin(c + 1, P.U, G);
+    if (u0 >= u1) return;
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    /* producer state (thread 0): next unit to load and its source block */
+    long long pu = u0, pblk = u0 % P.nblk;
+    if (tid == 0) {
+        for (int s = 0; s < STAGES - 1 && pu < u1; ++s) {
+            mbar_expect_tx(&full[s], SB * sizeof(float4));
+            tma_load_1d(&ring[s][0], unit_src(P, pblk), SB * sizeof(float4), &full[s]);
+            ++pu;
+            if (++pblk == P.nblk) pblk = 0;
+        }
+    }
+
+    const float self_u = P.self_sub ? rsqrt_approx(P.self_eps2) : 0.0f;
+    const float ke = (float)KE_D;
+
+    long long u = u0;
+    unsigned it = 0; /* units consumed so far by this CTA: stage = it % STAGES, parity = (it / STAGES) & 1 */
+    while (u < u1) {
+        const long long tile = u / P.nblk;
+        const long long b0 = u - tile * P.nblk;
+        const long long nrun = min(P.nblk - b0, u1 - u);
+        const long long tbase = tile * (long long)TT + tid;
+
+        u64 X[NPAIR], Y[NPAIR], Z[NPAIR];
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) {
+            const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
+            const float4 a = (i0 < P.nt) ? P.tgt[i0] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const float4 b = (i1 < P.nt) ? P.tgt[i1] : make_float4(0.f, 0.f, 0.f, 0.f);
+            X[p] = pk(a.x, b.x);
+            Y[p] = pk(a.y, b.y);
+            Z[p] = pk(a.z, b.z);
+        }
+        u64 RX[NPAIR], RY[NPAIR], RZ[NPAIR], RP[NPAIR];
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) RX[p] = RY[p] = RZ[p] = RP[p] = 0ull;
+
+        for (long long r = 0; r < nrun; ++r, ++it) {
+            const long long blk = b0 + r;
+            __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
+            if (tid == 0 && pu < u1) {
+                const int ps = (it + STAGES - 1) % STAGES;
+                mbar_expect_tx(&full[ps], SB * sizeof(float4));
+                tma_load_1d(&ring[ps][0], unit_src(P, pblk), SB * sizeof(float4), &full[ps]);
+                ++pu;
+                if (++pblk == P.nblk) pblk = 0;
+            }
+            const int st = it % STAGES;
+            mbar_wait(&full[st], (it / STAGES) & 1u);
+
+            u64 aX[NPAIR], aY[NPAIR], aZ[NPAIR], aP[NPAIR];
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p) aX[p] = aY[p] = aZ[p] = aP[p] = 0ull;
+            const float eps2 = (blk < P.sec[0].nblk) ? P.sec[0].eps2 : P.sec[1].eps2;
+            if (eps2 > 0.0f)
+                block_loop<false>(&ring[st][0], eps2, X, Y, Z, aX, aY, aZ, aP);
+            else
+                block_loop<true>(&ring[st][0], eps2, X, Y, Z, aX, aY, aZ, aP);
+            /* second accumulation level: flush the block sums into the running sums */
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p) {
+                RX[p] = add2(RX[p], aX[p]);
+                RY[p] = add2(RY[p], aY[p]);
+                RZ[p] = add2(RZ[p], aZ[p]);
+                RP[p] = add2(RP[p], aP[p]);
+            }
+        }
+
+        const bool whole = (b0 == 0 && nrun == P.nblk);
+        float4* wsl = P.ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT + tid;
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) {
+            float4 a, b;
+            upk(RX[p], a.x, b.x);
+            upk(RY[p], a.y, b.y);
+            upk(RZ[p], a.z, b.z);
+            upk(RP[p], a.w, b.w);
+            if (whole) {
+                const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
+                if (i0 < P.nt) {
+                    if (P.self_sub) a.w -= P.tgt[i0].w * self_u;
+                    P.out[i0] = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
+                }
+                if (i1 < P.nt) {
+                    if (P.self_sub) b.w -= P.tgt[i1].w * self_u;
+                    P.out[i1] = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
+                }
+            } else {
+                wsl[(2 * p) * THREADS] = a;
+                wsl[(2 * p + 1) * THREADS] = b;
+            }
+        }
+        u += nrun;
+    }
+}
+
+/* CTA whose unit range contains unit u (ranges are [floor(cU/G), floor((c+1)U/G)) ) */
+__device__ __forceinline__ long long cta_of(long long u, long long U, long long G)
+{
+    long long c = (long long)(((u64)u * (u64)G) / (u64)U);
+    while (c + 1 < G && unit_begin(c + 1, U, G) <= u) ++c;
+    while (c > 0 && unit_begin(c, U, G) > u) --c;
+    return c;
+}
+
+/* Tiles that were split between CTAs: sum their partials (fixed order, fp64), scale, write. */
+__global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P, const int G)
+{
+    const long long tile = blockIdx.x;
+    const long long uA = tile * P.nblk, uB = uA + P.nblk - 1;
+    const long long cA = cta_of(uA, P.U, G), cB = cta_of(uB, P.U, G);
+    if (cA == cB) return; /* one CTA had the whole tile and wrote it directly */
+    const int tid = threadIdx.x;
+    const float self_u = P.self_sub ? rsqrt_approx(P.self_eps2) : 0.0f;
+    for (int k = 0; k < TPT; ++k) {
+        const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
+        if (i >= P.nt) continue;
+        double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
+        for (long long c = cA; c <= cB; ++c) {
+            const long long c0 = unit_begin(c, P.U, G), c1 = unit_begin(c + 1, P.U, G);
+            if (c0 >= c1) continue;
+            const int slot = (c0 / P.nblk == tile) ? 0 : 1;
+            const float4 v = P.ws[((size_t)c * 2 + slot) * TT + (size_t)k * THREADS + tid];
+            ex += (double)v.x;
+            ey += (double)v.y;
+            ez += (double)v.z;
+            ph += (double)v.w;
+        }
+        if (P.self_sub) ph -= (double)(P.tgt[i].w * self_u);
+        P.out[i] = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
+    }
+}
+
+/* ------------------------------------------------------------------------------------------- */
+/* O(N) pack kernels                                                                            */
+/* ------------------------------------------------------------------------------------------- */
+__global__ void pack_charges_kernel(const float4* __restrict__ in, float4* __restrict__ out, long long n,
+                                    long long n_pad)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_pad) out[i] = (i < n) ? in[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+}
+
+/* 7-point degree-5 triangle rule (Radon): barycentric coordinate pattern (a, b, b) and weights,
+ * from the closed-form surds; g = 0: centroid, g = 1, 2: the two 3-point orbits. */
+__device__ __forceinline__ void quad7(int k, double& l0, double& l1, double& l2, double& w)
+{
+    const double s15 = sqrt(15.0);
+    if (k == 0) {
+        l0 = l1 = l2 = 1.0 / 3.0;
+        w = 9.0 / 40.0;
+        return;
+    }
+    const bool second = k > 3;
+    const double b = second ? (6.0 + s15) / 21.0 : (6.0 - s15) / 21.0;
+    const double a = 1.0 - 2.0 * b;
+    w = second ? (155.0 + s15) / 1200.0 : (155.0 - s15) / 1200.0;
+    const int j = (k - 1) % 3;
+    l0 = (j == 0) ? a : b;
+    l1 = (j == 1) ? a : b;
+    l2 = (j == 2) ? a : b;
+}
+
+/* one thread per panel: area and the 7 quadrature sources, derived in fp64, rounded once */
+__global__ void pack_panels_kernel(const float* __restrict__ verts, const float* __restrict__ sigma,
+                                   float4* __restrict__ src, double* __restrict__ area, long long np)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    double v[3][3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) v[j][d] = (double)verts[(p * 3 + j) * 3 + d];
+    const double ax = v[1][0] - v[0][0], ay = v[1][1] - v[0][1], az = v[1][2] - v[0][2];
+    const double bx = v[2][0] - v[0][0], by = v[2][1] - v[0][1], bz = v[2][2] - v[0][2];
+    const double cx = ay * bz - az * by, cy = az * bx - ax * bz, cz = ax * by - ay * bx;
+    const double A = 0.5 * sqrt(cx * cx + cy * cy + cz * cz);
+    area[p] = A;
+    const double sA = (double)sigma[p] * A;
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        double l0, l1, l2, w;
+        quad7(k, l0, l1, l2, w);
+        float4 o;
+        o.x = (float)(l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0]);
+        o.y = (float)(l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]);
+        o.z = (float)(l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]);
+        o.w = (float)(sA * w);
+        src[p * 7 + k] = o;
+    }
+}
+
+/* new sigma on the same geometry: rewrite the weights only */
+__global__ void set_sigma_kernel(const float* __restrict__ sigma, const double* __restrict__ area,
+                                 float4* __restrict__ src, long long np)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= np) return;
+    const double sA = (double)sigma[p] * area[p];
+#pragma unroll
+    for (int k = 0; k < 7; ++k) {
+        double l0, l1, l2, w;
+        quad7(k, l0, l1, l2, w);
+        src[p * 7 + k].w = (float)(sA * w);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------- */
+/* FP32 pipe probe (measurement aid)                                                            */
+/* ------------------------------------------------------------------------------------------- */
+constexpr int PROBE_CHAINS = 16;
+
+__global__ void __launch_bounds__(THREADS, CTAS_PER_SM) fma_probe_kernel(float* sink, long long iters, int mode)
+{
+    const float a = 1.0f + 1e-7f * threadIdx.x, b = 1e-9f * blockIdx.x;
+    if (mode == 0) {
+        float x[PROBE_CHAINS];
+#pragma unroll
+        for (int i = 0; i < PROBE_CHAINS; ++i) x[i] = (float)i;
+        for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < PROBE_CHAINS; ++i) x[i] = fmaf(x[i], a, b);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < PROBE_CHAINS; ++i) s += x[i];
+        if (s == 123.456f) sink[0] = s;
+    } else {
+        u64 x[PROBE_CHAINS / 2];
+        const u64 a2 = pk(a, a + 1e-7f), b2 = pk(b, b + 1e-9f);
+#pragma unroll
+        for (int i = 0; i < PROBE_CHAINS / 2; ++i) x[i] = pk((float)i, (float)i + 0.5f);
+        for (long long it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int i = 0; i < PROBE_CHAINS / 2; ++i) x[i] = fma2(x[i], a2, b2);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < PROBE_CHAINS / 2; ++i) {
+            float lo, hi;
+            upk(x[i], lo, hi);
+            s += lo + hi;
+        }
+        if (s == 123.456f) sink[0] = s;
+    }
+}
+
+inline long long ceil_div(long long a, long long b) { return (a + b - 1) / b; }
+
+} /* namespace */
+
+/* ------------------------------------------------------------------------------------------- */
+/* context and C ABI                                                                            */
+/* ------------------------------------------------------------------------------------------- */
+struct obem_ctx {
+    int device = 0;
+    int sm_count = 0;
+    int grid = 0;
+    float eps_pp = 0.f, eps_panel = 0.f;
+    /* charges */
+    float4* d_chg = nullptr;
+    long long chg_cap = 0; /* capacity in float4 (padded) */
+    long long n_chg = -1;
+    /* panels */
+    float4* d_psrc = nullptr;
+    double* d_area = nullptr;
+    long long pan_cap = 0; /* capacity in panels */
+    long long n_pan = -1;
+    /* split-tile workspace [grid][2][TT] */
+    float4* d_ws = nullptr;
+    float* d_sink = nullptr;
+    /* staging for the *_host entry points */
+    cudaStream_t hstream = nullptr;
+    void* d_stage[4] = {nullptr, nullptr, nullptr, nullptr};
+    size_t stage_cap[4] = {0, 0, 0, 0};
+    long long launches = 0;
+    int last_cuda = 0;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) ok = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+int cuda_fail(obem_ctx* c, cudaError_t e)
+{
+    if (c) c->last_cuda = (int)e;
+    cudaGetLastError(); /* clear the sticky-less error state */
+    return (e == cudaErrorMemoryAllocation) ? OBEM_ENOMEM : OBEM_ECUDA;
+}
+
+#define OBEM_CUDA(c, call)                                 \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return cuda_fail((c), e__); \
+    } while (0)
+
+bool aligned16(const void* p) { return (((uintptr_t)p) & 15u) == 0; }
+bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
+
+long long pad_sb(long long n) { return ceil_div(n, SB) * SB; }
+
+int grow_charges(obem_ctx* c, long long n)
+{
+    const long long need = pad_sb(n > 0 ? n : 1);
+    if (need <= c->chg_cap) return OBEM_OK;
+    float4* p = nullptr;
+    OBEM_CUDA(c, cudaMalloc(&p, (size_t)need * sizeof(float4)));
+    if (c->d_chg) cudaFree(c->d_chg);
+    c->d_chg = p;
+    c->chg_cap = need;
+    return OBEM_OK;
+}
+
+int grow_panels(obem_ctx* c, long long np)
+{
+    const long long need = np > 0 ? np : 1;
+    if (need <= c->pan_cap) return OBEM_OK;
+    float4* p = nullptr;
+    double* a = nullptr;
+    OBEM_CUDA(c, cudaMalloc(&p, (size_t)pad_sb(need * 7) * sizeof(float4)));
+    cudaError_t e = cudaMalloc(&a, (size_t)need * sizeof(double));
+    if (e != cudaSuccess) {
+        cudaFree(p);
+        return cuda_fail(c, e);
+    }
+    if (c->d_psrc) cudaFree(c->d_psrc);
+    if (c->d_area) cudaFree(c->d_area);
+    c->d_psrc = p;
+    c->d_area = a;
+    c->pan_cap = need;
+    return OBEM_OK;
+}
+
+int grow_stage(obem_ctx* c, int i, size_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    if (bytes <= c->stage_cap[i]) return OBEM_OK;
+    void* p = nullptr;
+    OBEM_CUDA(c, cudaMalloc(&p, bytes));
+    if (c->d_stage[i]) cudaFree(c->d_stage[i]);
+    c->d_stage[i] = p;
+    c->stage_cap[i] = bytes;
+    return OBEM_OK;
+}
+
+/* the evaluation proper: targets tgt[0..nt) -> out[0..nt) */
+int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, bool at_charges,
+                cudaStream_t st)
+{
+    if (flags & ~(OBEM_NBODY | OBEM_PANELS)) return OBEM_EINVAL;
+    if ((flags & OBEM_NBODY) && c->n_chg < 0) return OBEM_ESTATE;
+    if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
+    if (nt == 0) return OBEM_OK;
+
+    EvalParams P;
+    int ns = 0;
+    P.sec[0].src = P.sec[1].src = nullptr;
+    P.sec[0].nblk = P.sec[1].nblk = 0;
+    P.sec[0].eps2 = P.sec[1].eps2 = 0.f;
+    P.self_sub = 0;
+    P.self_eps2 = 0.f;
+    if ((flags & OBEM_NBODY) && c->n_chg > 0) {
+        P.sec[ns].src = c->d_chg;
+        P.sec[ns].nblk = ceil_div(c->n_chg, SB);
+        P.sec[ns].eps2 = c->eps_pp * c->eps_pp;
+        /* reading A3: the self term is excluded by index.  With softening it is the exactly known
+         * amount q_i * rsqrt(eps^2) in phi (and exactly 0 in E): the kernels subtract it.  Without
+         * softening the zero-distance guard (reading A4) already drops it. */
+        if (at_charges && P.sec[ns].eps2 > 0.f) {
+            P.self_sub = 1;
+            P.self_eps2 = P.sec[ns].eps2;
+        }
+        ++ns;
+    }
+    if ((flags & OBEM_PANELS) && c->n_pan > 0) {
+        P.sec[ns].src = c->d_psrc;
+        P.sec[ns].nblk = ceil_div(c->n_pan * 7, SB);
+        P.sec[ns].eps2 = c->eps_panel * c->eps_panel;
+        ++ns;
+    }
+    if (ns == 0) {
+        OBEM_CUDA(c, cudaMemsetAsync(out, 0, (size_t)nt * sizeof(float4), st));
+        return OBEM_OK;
+    }
+    P.nblk = P.sec[0].nblk + P.sec[1].nblk;
+    P.tgt = tgt;
+    P.nt = nt;
+    P.ntiles = ceil_div(nt, TT);
+    P.U = P.ntiles * P.nblk;
+    P.out = out;
+    P.ws = c->d_ws;
+
+    obem_eval_kernel<<<c->grid, THREADS, 0, st>>>(P);
+    OBEM_CUDA(c, cudaGetLastError());
+    obem_fixup_kernel<<<(unsigned)P.ntiles, THREADS, 0, st>>>(P, c->grid);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 2;
+    return OBEM_OK;
+}
+
+} /* namespace */
+
+extern "C" {
+
+int obem_create(obem_ctx** out, int device)
+{
+    if (!out) return OBEM_EINVAL;
+    *out = nullptr;
+    if (device < 0) return OBEM_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) {
+        cudaGetLastError();
+        return OBEM_ECUDA;
+    }
+    DeviceGuard g(device);
+    if (!g.ok) return OBEM_ECUDA;
+    obem_ctx* c = new (std::nothrow) obem_ctx();
+    if (!c) return OBEM_ENOMEM;
+    c->device = device;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) {
+        delete c;
+        return OBEM_ECUDA;
+    }
+    c->sm_count = prop.multiProcessorCount;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel, THREADS, 0);
+    if (e != cudaSuccess || per_sm < 1) {
+        /* no sm_100a code for this device, or the kernel cannot be resident */
+        cudaGetLastError();
+        delete c;
+        return OBEM_ECUDA;
+    }
+    if (per_sm > CTAS_PER_SM) per_sm = CTAS_PER_SM;
+    c->grid = c->sm_count * per_sm;
+    e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_sink, 256);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking);
+    if (e != cudaSuccess) {
+        int rc = cuda_fail(nullptr, e);
+        obem_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return OBEM_OK;
+}
+
+int obem_destroy(obem_ctx* c)
+{
+    if (!c) return OBEM_OK;
+    DeviceGuard g(c->device);
+    cudaDeviceSynchronize();
+    if (c->d_chg) cudaFree(c->d_chg);
+    if (c->d_psrc) cudaFree(c->d_psrc);
+    if (c->d_area) cudaFree(c->d_area);
+    if (c->d_ws) cudaFree(c->d_ws);
+    if (c->d_sink) cudaFree(c->d_sink);
+    for (int i = 0; i < 4; ++i)
+        if (c->d_stage[i]) cudaFree(c->d_stage[i]);
+    if (c->hstream) cudaStreamDestroy(c->hstream);
+    cudaGetLastError();
+    delete c;
+    return OBEM_OK;
+}
+
+int obem_reserve(obem_ctx* c, int64_t n_charges, int64_t n_panels)
+{
+    if (!c || n_charges < 0 || n_panels < 0) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    int rc = grow_charges(c, n_charges);
+    if (rc != OBEM_OK) return rc;
+    return grow_panels(c, n_panels);
+}
+
+int obem_set_softening(obem_ctx* c, float eps_pp_m, float eps_panel_m)
+{
+    if (!c) return OBEM_EINVAL;
+    if (!(eps_pp_m >= 0.f) || !(eps_panel_m >= 0.f) || isinf(eps_pp_m) || isinf(eps_panel_m)) return OBEM_EINVAL;
+    c->eps_pp = eps_pp_m;
+    c->eps_panel = eps_panel_m;
+    return OBEM_OK;
+}
+
+int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int64_t n_panels, void* cuda_stream)
+{
+    if (!c || n_panels < 0) return OBEM_EINVAL;
+    if (n_panels > 0 && (!d_verts || !d_sigma || !aligned4(d_verts) || !aligned4(d_sigma))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = grow_panels(c, n_panels);
+    if (rc != OBEM_OK) return rc;
+    if (n_panels > 0) {
+        const long long ns = n_panels * 7, ns_pad = pad_sb(ns);
+        if (ns_pad > ns)
+            OBEM_CUDA(c, cudaMemsetAsync(c->d_psrc + ns, 0, (size_t)(ns_pad - ns) * sizeof(float4), st));
+        pack_panels_kernel<<<(unsigned)ceil_div(n_panels, 128), 128, 0, st>>>(d_verts, d_sigma, c->d_psrc,
+                                                                              c->d_area, n_panels);
+        OBEM_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    c->n_pan = n_panels;
+    return OBEM_OK;
+}
+
+int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cuda_stream)
+{
+    if (!c || n_panels < 0) return OBEM_EINVAL;
+    if (c->n_pan < 0) return OBEM_ESTATE;
+    if (n_panels != c->n_pan) return OBEM_EINVAL;
+    if (n_panels > 0 && (!d_sigma || !aligned4(d_sigma))) return OBEM_EINVAL;
+    if (n_panels == 0) return OBEM_OK;
+    DeviceGuard g(c->device);
+    set_sigma_kernel<<<(unsigned)ceil_div(n_panels, 128), 128, 0, (cudaStream_t)cuda_stream>>>(
+        d_sigma, c->d_area, c->d_psrc, n_panels);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return OBEM_OK;
+}
+
+int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_stream)
+{
+    if (!c || n < 0) return OBEM_EINVAL;
+    if (n > 0 && (!d_xyzq || !aligned16(d_xyzq))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    int rc = grow_charges(c, n);
+    if (rc != OBEM_OK) return rc;
+    if (n > 0) {
+        const long long n_pad = pad_sb(n);
+        pack_charges_kernel<<<(unsigned)ceil_div(n_pad, 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+            (const float4*)d_xyzq, c->d_chg, n, n_pad);
+        OBEM_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    c->n_chg = n;
+    return OBEM_OK;
+}
+
+int obem_eval_at_charges_range(obem_ctx* c, int64_t first, int64_t count, float* d_out, unsigned flags,
+                               void* cuda_stream)
+{
+    if (!c || first < 0 || count < 0) return OBEM_EINVAL;
+    if (c->n_chg < 0) return OBEM_ESTATE;
+    if (first + count > c->n_chg) return OBEM_EINVAL;
+    if (count > 0 && (!d_out || !aligned16(d_out))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    return eval_common(c, c->d_chg + first, count, (float4*)d_out, flags, true, (cudaStream_t)cuda_stream);
+}
+
+int obem_eval_at_charges(obem_ctx* c, float* d_out, unsigned flags, void* cuda_stream)
+{
+    if (!c) return OBEM_EINVAL;
+    if (c->n_chg < 0) return OBEM_ESTATE;
+    return obem_eval_at_charges_range(c, 0, c->n_chg, d_out, flags, cuda_stream);
+}
+
+int obem_eval_at_points(obem_ctx* c, const float* d_pts, int64_t m, float* d_out, unsigned flags, void* cuda_stream)
+{
+    if (!c || m < 0) return OBEM_EINVAL;
+    if (m > 0 && (!d_pts || !d_out || !aligned16(d_pts) || !aligned16(d_out))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    return eval_common(c, (const float4*)d_pts, m, (float4*)d_out, flags, false, (cudaStream_t)cuda_stream);
+}
+
+static int host_set_panels(obem_ctx* c, const float* h_verts, const float* h_sigma, int64_t np)
+{
+    if (!h_verts) return OBEM_OK; /* keep the panels already set */
+    if (np < 0 || (np > 0 && !h_sigma)) return OBEM_EINVAL;
+    int rc = grow_stage(c, 1, (size_t)np * 9 * sizeof(float));
+    if (rc == OBEM_OK) rc = grow_stage(c, 2, (size_t)np * sizeof(float));
+    if (rc != OBEM_OK) return rc;
+    if (np > 0) {
+        OBEM_CUDA(c, cudaMemcpyAsync(c->d_stage[1], h_verts, (size_t)np * 9 * sizeof(float), cudaMemcpyHostToDevice,
+                                     c->hstream));
+        OBEM_CUDA(c, cudaMemcpyAsync(c->d_stage[2], h_sigma, (size_t)np * sizeof(float), cudaMemcpyHostToDevice,
+                                     c->hstream));
+    }
+    return obem_set_panels(c, (const float*)c->d_stage[1], (const float*)c->d_stage[2], np, c->hstream);
+}
+
+int obem_field_at_charges_host(obem_ctx* c, const float* h_xyzq, int64_t n, const float* h_verts,
+                               const float* h_sigma, int64_t n_panels, float* h_out, unsigned flags)
+{
+    if (!c || n < 0 || (n > 0 && (!h_xyzq || !h_out))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    int rc = host_set_panels(c, h_verts, h_sigma, n_panels);
+    if (rc != OBEM_OK) return rc;
+    rc = grow_stage(c, 0, (size_t)n * sizeof(float4));
+    if (rc == OBEM_OK) rc = grow_stage(c, 3, (size_t)n * sizeof(float4));
+    if (rc != OBEM_OK) return rc;
+    if (n > 0)
+        OBEM_CUDA(c, cudaMemcpyAsync(c->d_stage[0], h_xyzq, (size_t)n * sizeof(float4), cudaMemcpyHostToDevice,
+                                     c->hstream));
+    rc = obem_set_charges(c, (const float*)c->d_stage[0], n, c->hstream);
+    if (rc != OBEM_OK) return rc;
+    rc = obem_eval_at_charges(c, (float*)c->d_stage[3], flags, c->hstream);
+    if (rc != OBEM_OK) return rc;
+    if (n > 0)
+        OBEM_CUDA(c, cudaMemcpyAsync(h_out, c->d_stage[3], (size_t)n * sizeof(float4), cudaMemcpyDeviceToHost,
+                                     c->hstream));
+    OBEM_CUDA(c, cudaStreamSynchronize(c->hstream));
+    return OBEM_OK;
+}
+
+int obem_field_at_points_host(obem_ctx* c, const float* h_pts, int64_t m, const float* h_verts, const float* h_sigma,
+                              int64_t n_panels, float* h_out, unsigned flags)
+{
+    if (!c || m < 0 || (m > 0 && (!h_pts || !h_out))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    int rc = host_set_panels(c, h_verts, h_sigma, n_panels);
+    if (rc != OBEM_OK) return rc;
+    rc = grow_stage(c, 0, (size_t)m * sizeof(float4));
+    if (rc == OBEM_OK) rc = grow_stage(c, 3, (size_t)m * sizeof(float4));
+    if (rc != OBEM_OK) return rc;
+    if (m > 0)
+        OBEM_CUDA(c, cudaMemcpyAsync(c->d_stage[0], h_pts, (size_t)m * sizeof(float4), cudaMemcpyHostToDevice,
+                                     c->hstream));
+    rc = obem_eval_at_points(c, (const float*)c->d_stage[0], m, (float*)c->d_stage[3], flags, c->hstream);
+    if (rc != OBEM_OK) return rc;
+    if (m > 0)
+        OBEM_CUDA(c, cudaMemcpyAsync(h_out, c->d_stage[3], (size_t)m * sizeof(float4), cudaMemcpyDeviceToHost,
+                                     c->hstream));
+    OBEM_CUDA(c, cudaStreamSynchronize(c->hstream));
+    return OBEM_OK;
+}
+
+int64_t obem_n_charges(const obem_ctx* c) { return c ? c->n_chg : -1; }
+int64_t obem_n_panels(const obem_ctx* c) { return c ? c->n_pan : -1; }
+int obem_sm_count(const obem_ctx* c) { return c ? c->sm_count : 0; }
+int obem_grid_size(const obem_ctx* c) { return c ? c->grid : 0; }
+int64_t obem_kernel_launches(const obem_ctx* c) { return c ? c->launches : 0; }
+int obem_last_cuda_error(const obem_ctx* c) { return c ? c->last_cuda : 0; }
+
+const char* obem_status_string(int status)
+{
+    switch (status) {
+    case OBEM_OK: return "OBEM_OK";
+    case OBEM_EINVAL: return "OBEM_EINVAL: null, negative, misaligned or inconsistent argument";
+    case OBEM_ESTATE: return "OBEM_ESTATE: evaluate/update before the sources were set";
+    case OBEM_ECUDA: return "OBEM_ECUDA: a CUDA call failed (see obem_last_cuda_error)";
+    case OBEM_ENOMEM: return "OBEM_ENOMEM: device allocation failed";
+    default: return "unknown obem_status";
+    }
+}
+
+int obem_get_panel_sources(obem_ctx* c, float* d_out, void* cuda_stream)
+{
+    if (!c) return OBEM_EINVAL;
+    if (c->n_pan < 0) return OBEM_ESTATE;
+    if (c->n_pan == 0) return OBEM_OK;
+    if (!d_out || !aligned16(d_out)) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    OBEM_CUDA(c, cudaMemcpyAsync(d_out, c->d_psrc, (size_t)c->n_pan * 7 * sizeof(float4), cudaMemcpyDeviceToDevice,
+                                 (cudaStream_t)cuda_stream));
+    return OBEM_OK;
+}
+
+int obem_fma_peak_probe(obem_ctx* c, int mode, int64_t iters, double* flops_out, void* cuda_stream)
+{
+    if (!c || iters < 0 || (mode != 0 && mode != 1)) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    fma_probe_kernel<<<c->grid, THREADS, 0, (cudaStream_t)cuda_stream>>>(c->d_sink, iters, mode);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    if (flops_out) *flops_out = 2.0 * PROBE_CHAINS * (double)iters * THREADS * (double)c->grid;
+    return OBEM_OK;
+}
+
+} /* extern "C" */
