@@ -32,13 +32,33 @@ namespace {
 
 typedef unsigned long long u64;
 
-constexpr int THREADS = 256;          /* threads per CTA of the evaluation kernel                 */
-constexpr int TPT = 8;                /* targets per thread                                        */
+/* Tuning knobs (overridable with -D for sweeps; the defaults are the measured best) */
+#ifndef OBEM_THREADS
+#define OBEM_THREADS 256
+#endif
+#ifndef OBEM_TPT
+#define OBEM_TPT 8
+#endif
+#ifndef OBEM_CTAS
+#define OBEM_CTAS 1
+#endif
+#ifndef OBEM_UNR
+#define OBEM_UNR 4
+#endif
+#ifndef OBEM_DEPTH
+#define OBEM_DEPTH 4
+#endif
+constexpr int THREADS = OBEM_THREADS;  /* threads per CTA of the evaluation kernel                 */
+constexpr int TPT = OBEM_TPT;         /* targets per thread                                        */
 constexpr int NPAIR = TPT / 2;        /* packed f32x2 target pairs per thread                      */
-constexpr int TT = THREADS * TPT;     /* targets per tile (2048)                                   */
+constexpr int TT = THREADS * TPT;     /* targets per tile                                          */
 constexpr int SB = 256;               /* sources per shared-memory block (4 KiB)                   */
 constexpr int STAGES = 4;             /* depth of the TMA ring                                     */
-constexpr int CTAS_PER_SM = 2;
+constexpr int CTAS_PER_SM = OBEM_CTAS;
+constexpr int UNR = OBEM_UNR;         /* sources per unrolled inner-loop trip                      */
+constexpr int DEPTH = OBEM_DEPTH;     /* software-pipeline distance (work items) between the rsqrt
+                                         of an item and its use                                     */
+static_assert(TPT % 2 == 0 && SB % UNR == 0, "bad tuning knobs");
 
 /* k_e = 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), reading A7 */
 constexpr double KE_D = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12);
@@ -50,6 +70,14 @@ __device__ __forceinline__ u64 pk(float lo, float hi)
 {
     u64 r;
     asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+/* same, but opaque to the optimiser: the pair is built once and kept (used for loop-invariant targets,
+ * which the compiler would otherwise re-pack from their float4 registers inside the hot loop) */
+__device__ __forceinline__ u64 pk_keep(float lo, float hi)
+{
+    u64 r;
+    asm volatile("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
     return r;
 }
 __device__ __forceinline__ void upk(u64 v, float& lo, float& hi)
@@ -130,22 +158,27 @@ __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem
 /* evaluation kernel                                                                            */
 /* ------------------------------------------------------------------------------------------- */
 struct Section {
-    const float4* src; /* packed sources (x, y, z, weight), padded to a multiple of SB with weight 0 */
-    long long nblk;    /* number of SB-blocks                                                        */
-    float eps2;        /* softening^2 of this section                                                */
+    const float4* src; /* packed sources, SB float4 per block (layout by kind), padded with weight-0 entries */
+    long long nblk;    /* number of SB-blocks                                                            */
+    float eps2;        /* softening^2 of this section                                                    */
+    int kind;          /* KIND_POINTS: SB point sources (x, y, z, w) per block.
+                          KIND_PANELS: SB/8 panels per block, each 8 float4: a frame origin c (x, y, z, -)
+                          followed by 7 quadrature sources (x - c_x, y - c_y, z - c_z, w) in that frame. */
 };
+constexpr int KIND_POINTS = 0, KIND_PANELS = 1;
+constexpr int PANELS_PER_BLOCK = SB / 8;
 
 struct EvalParams {
     Section sec[2];
-    long long nblk;   /* sec[0].nblk + sec[1].nblk                                   */
+    long long nblk;       /* sec[0].nblk + sec[1].nblk                                                   */
     const float4* tgt;
-    long long nt;     /* targets                                                     */
-    long long ntiles; /* ceil(nt / TT)                                               */
-    long long U;      /* work units = ntiles * nblk                                  */
-    float4* out;      /* [nt]                                                        */
-    float4* ws;       /* [grid][2][TT] partial sums of split tiles                   */
-    int self_sub;     /* 1: subtract the target's own softened phi term (reading A3) */
-    float self_eps2;
+    long long nt;         /* targets                                                                     */
+    long long ntiles;     /* ceil(nt / TT)                                                               */
+    long long U;          /* work units = ntiles * nblk                                                  */
+    float4* out;          /* [nt]                                                                        */
+    float4* ws;           /* [grid][2][TT] partial sums of split tiles                                   */
+    long long self_first; /* >= 0: target i IS point source (self_first + i) of sec[0] and is excluded
+                             from its own sum by index (reading A3); -1: no exclusion                    */
 };
 
 /* first work unit of CTA c: floor(c * U / G) */
@@ -155,45 +188,141 @@ __device__ __forceinline__ long long unit_begin(long long c, long long U, long l
 }
 
 /*
- * One shared-memory block of SB sources against the thread's 8 targets.
- * Per source and target pair: 3 FADD2 (d = r_t - r_s), 3 FFMA2 (r2 = d.d + eps^2), 2 MUFU.RSQ,
- * FMUL2 (t = w u), FADD2 (phi += t), FMUL2 (u^2), FMUL2 (s = t u^2), 3 FFMA2 (E += s d).
+ * The interaction body, split in two halves so that the loops below can software-pipeline it:
+ *   front: 3 FADD2 (d = r_t - r_s), 3 FFMA2 (r2 = d.d + eps^2), 2 MUFU.RSQ
+ *   back : FMUL2 (t = w u), FADD2 (phi += t), FMUL2 (u^2), FMUL2 (s = t u^2), 3 FFMA2 (E += s d)
+ * = 13 packed FP32-pipe instructions + 2 MUFU per (source, target pair).
  * GUARD (eps = 0 only): a source at zero distance contributes 0 (reading A4).
  */
+template <bool GUARD>
+__device__ __forceinline__ void item_front(u64& dx, u64& dy, u64& dz, u64& u, const u64 tx, const u64 ty,
+                                           const u64 tz, const float sx, const float sy, const float sz,
+                                           const u64 e2)
+{
+    dx = sub2(tx, pk(sx, sx));
+    dy = sub2(ty, pk(sy, sy));
+    dz = sub2(tz, pk(sz, sz));
+    u64 r2 = fma2(dx, dx, e2);
+    r2 = fma2(dy, dy, r2);
+    r2 = fma2(dz, dz, r2);
+    float r2l, r2h;
+    upk(r2, r2l, r2h);
+    float ul = rsqrt_approx(r2l);
+    float uh = rsqrt_approx(r2h);
+    if (GUARD) {
+        ul = (r2l > 0.0f) ? ul : 0.0f;
+        uh = (r2h > 0.0f) ? uh : 0.0f;
+    }
+    u = pk(ul, uh);
+}
+__device__ __forceinline__ void item_back(const u64 dx, const u64 dy, const u64 dz, const u64 u, const u64 w,
+                                          u64& ax, u64& ay, u64& az, u64& ap)
+{
+    const u64 t = mul2(u, w);
+    ap = add2(ap, t);
+    const u64 u2 = mul2(u, u);
+    const u64 sE = mul2(t, u2);
+    ax = fma2(sE, dx, ax);
+    ay = fma2(sE, dy, ay);
+    az = fma2(sE, dz, az);
+}
+
+/* One block of SB point sources against the thread's TPT targets (KIND_POINTS). */
 template <bool GUARD>
 __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                            u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
 {
     const u64 e2 = pk(eps2, eps2);
-#pragma unroll 2
-    for (int j = 0; j < SB; ++j) {
-        const float4 q = s[j]; /* warp-uniform address: one broadcast LDS.128 */
-        const u64 sx = pk(q.x, q.x), sy = pk(q.y, q.y), sz = pk(q.z, q.z), sw = pk(q.w, q.w);
+    constexpr int K = UNR * NPAIR; /* work items (source, target pair) per trip */
+#pragma unroll 1
+    for (int j0 = 0; j0 < SB; j0 += UNR) {
+        float4 q[UNR];
+#pragma unroll
+        for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j]; /* warp-uniform address: broadcast LDS.128 */
+        u64 dX[K], dY[K], dZ[K], U[K];
+        /* software pipeline over the K items of the trip: item k's distance + rsqrt are issued DEPTH
+         * items before its accumulation, so the MUFU latency is covered by independent FFMA2 work */
+#pragma unroll
+        for (int k = 0; k < K + DEPTH; ++k) {
+            if (k < K) {
+                const int j = k / NPAIR, p = k % NPAIR;
+                item_front<GUARD>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+            }
+            if (k >= DEPTH) {
+                const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
+                item_back(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
+            }
+        }
+    }
+}
+
+/*
+ * One block of SB/8 panels (KIND_PANELS).  Each panel carries its own frame: the targets are shifted
+ * into it once per panel (3 FADD2 per pair, amortised over 7 sources), and the 7 quadrature points are
+ * stored relative to the frame origin.  Why: a quadrature point rounded to fp32 in GLOBAL coordinates
+ * is off by up to half an ulp of the coordinate (7e-12 m at 0.2 mm, 1e-10 m at 3 mm), which is a
+ * relative error of 1e-4..1e-2 in the field of a source 10-100 nm away; relative to the panel's own
+ * centroid the same rounding is ~100x smaller, and t - c is exact for nearby targets (Sterbenz).
+ */
+template <bool GUARD>
+__device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
+                                           const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
+                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
+{
+    const u64 e2 = pk(eps2, eps2);
+    constexpr int K = 7 * NPAIR;
+#pragma unroll 1
+    for (int pp = 0; pp < PANELS_PER_BLOCK; ++pp) {
+        const float4 o = s[pp * 8];
+        float4 q[7];
+#pragma unroll
+        for (int j = 0; j < 7; ++j) q[j] = s[pp * 8 + 1 + j];
+        u64 TX[NPAIR], TY[NPAIR], TZ[NPAIR];
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
-            const u64 dx = sub2(X[p], sx);
-            const u64 dy = sub2(Y[p], sy);
-            const u64 dz = sub2(Z[p], sz);
-            u64 r2 = fma2(dx, dx, e2);
-            r2 = fma2(dy, dy, r2);
-            r2 = fma2(dz, dz, r2);
-            float r2l, r2h;
-            upk(r2, r2l, r2h);
-            float ul = rsqrt_approx(r2l);
-            float uh = rsqrt_approx(r2h);
-            if (GUARD) {
-                ul = (r2l > 0.0f) ? ul : 0.0f;
-                uh = (r2h > 0.0f) ? uh : 0.0f;
+            TX[p] = sub2(X[p], pk(o.x, o.x));
+            TY[p] = sub2(Y[p], pk(o.y, o.y));
+            TZ[p] = sub2(Z[p], pk(o.z, o.z));
+        }
+        u64 dX[K], dY[K], dZ[K], U[K];
+#pragma unroll
+        for (int k = 0; k < K + DEPTH; ++k) {
+            if (k < K) {
+                const int j = k / NPAIR, p = k % NPAIR;
+                item_front<GUARD>(dX[k], dY[k], dZ[k], U[k], TX[p], TY[p], TZ[p], q[j].x, q[j].y, q[j].z, e2);
             }
-            const u64 u = pk(ul, uh);
-            const u64 t = mul2(u, sw);
-            aP[p] = add2(aP[p], t);
-            const u64 u2 = mul2(u, u);
-            const u64 sE = mul2(t, u2);
-            aX[p] = fma2(sE, dx, aX[p]);
-            aY[p] = fma2(sE, dy, aY[p]);
-            aZ[p] = fma2(sE, dz, aZ[p]);
+            if (k >= DEPTH) {
+                const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
+                item_back(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
+            }
+        }
+    }
+}
+
+/*
+ * The rare diagonal block: a block of point sources that contains some of this tile's own targets
+ * (evaluation at the charges).  Eq (3.8)'s p != p' is applied BY INDEX: the weight of source j is
+ * zeroed for the target whose source index is j.  selfrel[k] = (source index of target slot k) - (first
+ * source index of the block); always guarded (d = 0 there).  Simple loop: it runs for TT/SB of the
+ * blocks of a tile only.
+ */
+__device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
+                                             const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
+                                             u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR],
+                                             const long long selfrel0, const int selfrel_stride)
+{
+    const u64 e2 = pk(eps2, eps2);
+#pragma unroll 1
+    for (int j = 0; j < SB; ++j) {
+        const float4 q = s[j];
+#pragma unroll
+        for (int p = 0; p < NPAIR; ++p) {
+            u64 dx, dy, dz, u;
+            item_front<true>(dx, dy, dz, u, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+            const float wl = (selfrel0 + (long long)(2 * p) * selfrel_stride == j) ? 0.0f : q.w;
+            const float wh = (selfrel0 + (long long)(2 * p + 1) * selfrel_stride == j) ? 0.0f : q.w;
+            item_back(dx, dy, dz, u, pk(wl, wh), aX[p], aY[p], aZ[p], aP[p]);
         }
     }
 }
@@ -230,7 +359,6 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
         }
     }
 
-    const float self_u = P.self_sub ? rsqrt_approx(P.self_eps2) : 0.0f;
     const float ke = (float)KE_D;
 
     long long u = u0;
@@ -245,15 +373,21 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
             const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
-            const float4 a = (i0 < P.nt) ? P.tgt[i0] : make_float4(0.f, 0.f, 0.f, 0.f);
-            const float4 b = (i1 < P.nt) ? P.tgt[i1] : make_float4(0.f, 0.f, 0.f, 0.f);
-            X[p] = pk(a.x, b.x);
-            Y[p] = pk(a.y, b.y);
-            Z[p] = pk(a.z, b.z);
+            /* scalar loads on purpose: a 128-bit load pins x,y,z,w to consecutive registers and ptxas then
+             * re-pairs (x_a, x_b) with MOVs inside the hot loop */
+            const float* ta = (const float*)(P.tgt + i0);
+            const float* tb = (const float*)(P.tgt + i1);
+            const bool va = i0 < P.nt, vb = i1 < P.nt;
+            X[p] = pk_keep(va ? __ldg(ta + 0) : 0.f, vb ? __ldg(tb + 0) : 0.f);
+            Y[p] = pk_keep(va ? __ldg(ta + 1) : 0.f, vb ? __ldg(tb + 1) : 0.f);
+            Z[p] = pk_keep(va ? __ldg(ta + 2) : 0.f, vb ? __ldg(tb + 2) : 0.f);
         }
         u64 RX[NPAIR], RY[NPAIR], RZ[NPAIR], RP[NPAIR];
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) RX[p] = RY[p] = RZ[p] = RP[p] = 0ull;
+
+        /* source-index range of this tile's own targets inside sec[0] (evaluation at the charges) */
+        const long long self_lo = (P.self_first >= 0) ? P.self_first + tile * (long long)TT : -1;
 
         for (long long r = 0; r < nrun; ++r, ++it) {
             const long long blk = b0 + r;
@@ -271,11 +405,22 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             u64 aX[NPAIR], aY[NPAIR], aZ[NPAIR], aP[NPAIR];
 #pragma unroll
             for (int p = 0; p < NPAIR; ++p) aX[p] = aY[p] = aZ[p] = aP[p] = 0ull;
-            const float eps2 = (blk < P.sec[0].nblk) ? P.sec[0].eps2 : P.sec[1].eps2;
-            if (eps2 > 0.0f)
-                block_loop<false>(&ring[st][0], eps2, X, Y, Z, aX, aY, aZ, aP);
-            else
-                block_loop<true>(&ring[st][0], eps2, X, Y, Z, aX, aY, aZ, aP);
+            const bool first_sec = blk < P.sec[0].nblk;
+            const float eps2 = first_sec ? P.sec[0].eps2 : P.sec[1].eps2;
+            const int kind = first_sec ? P.sec[0].kind : P.sec[1].kind;
+            const float4* sblk = &ring[st][0];
+            if (kind == KIND_PANELS) {
+                if (eps2 > 0.0f)
+                    panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                else
+                    panel_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            } else if (first_sec && self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo) {
+                self_block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, self_lo + tid - blk * SB, THREADS);
+            } else if (eps2 > 0.0f) {
+                block_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            } else {
+                block_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            }
             /* second accumulation level: flush the block sums into the running sums */
 #pragma unroll
             for (int p = 0; p < NPAIR; ++p) {
@@ -297,14 +442,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             upk(RP[p], a.w, b.w);
             if (whole) {
                 const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
-                if (i0 < P.nt) {
-                    if (P.self_sub) a.w -= P.tgt[i0].w * self_u;
-                    P.out[i0] = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
-                }
-                if (i1 < P.nt) {
-                    if (P.self_sub) b.w -= P.tgt[i1].w * self_u;
-                    P.out[i1] = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
-                }
+                if (i0 < P.nt) P.out[i0] = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
+                if (i1 < P.nt) P.out[i1] = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
             } else {
                 wsl[(2 * p) * THREADS] = a;
                 wsl[(2 * p + 1) * THREADS] = b;
@@ -331,7 +470,6 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
     const long long cA = cta_of(uA, P.U, G), cB = cta_of(uB, P.U, G);
     if (cA == cB) return; /* one CTA had the whole tile and wrote it directly */
     const int tid = threadIdx.x;
-    const float self_u = P.self_sub ? rsqrt_approx(P.self_eps2) : 0.0f;
     for (int k = 0; k < TPT; ++k) {
         const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
         if (i >= P.nt) continue;
@@ -346,7 +484,6 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
             ez += (double)v.z;
             ph += (double)v.w;
         }
-        if (P.self_sub) ph -= (double)(P.tgt[i].w * self_u);
         P.out[i] = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
     }
 }
@@ -354,11 +491,14 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
 /* ------------------------------------------------------------------------------------------- */
 /* O(N) pack kernels                                                                            */
 /* ------------------------------------------------------------------------------------------- */
+constexpr float PAD_FAR = 1.0e15f;
+
 __global__ void pack_charges_kernel(const float4* __restrict__ in, float4* __restrict__ out, long long n,
                                     long long n_pad)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n_pad) out[i] = (i < n) ? in[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    /* padding: weight 0, parked far away so that it is never at zero distance from a target */
+    if (i < n_pad) out[i] = (i < n) ? in[i] : make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
 }
 
 /* 7-point degree-5 triangle rule (Radon): barycentric coordinate pattern (a, b, b) and weights,
@@ -381,12 +521,21 @@ __device__ __forceinline__ void quad7(int k, double& l0, double& l1, double& l2,
     l2 = (j == 2) ? a : b;
 }
 
-/* one thread per panel: area and the 7 quadrature sources, derived in fp64, rounded once */
+/* one thread per panel slot (np_pad of them): area, frame origin and the 7 quadrature sources, derived in
+ * fp64 and rounded once.  Frame origin c = the centroid rounded to fp32; sources are stored as
+ * (x_k - c) in fp32 (see panel_loop).  Slots >= np are padding (weight 0, parked far away). */
 __global__ void pack_panels_kernel(const float* __restrict__ verts, const float* __restrict__ sigma,
-                                   float4* __restrict__ src, double* __restrict__ area, long long np)
+                                   float4* __restrict__ src, double* __restrict__ area, long long np,
+                                   long long np_pad)
 {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= np) return;
+    if (p >= np_pad) return;
+    if (p >= np) {
+        src[p * 8] = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int k = 0; k < 7; ++k) src[p * 8 + 1 + k] = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+        return;
+    }
     double v[3][3];
 #pragma unroll
     for (int j = 0; j < 3; ++j)
@@ -398,16 +547,22 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
     const double A = 0.5 * sqrt(cx * cx + cy * cy + cz * cz);
     area[p] = A;
     const double sA = (double)sigma[p] * A;
+    float4 o;
+    o.x = (float)((v[0][0] + v[1][0] + v[2][0]) / 3.0);
+    o.y = (float)((v[0][1] + v[1][1] + v[2][1]) / 3.0);
+    o.z = (float)((v[0][2] + v[1][2] + v[2][2]) / 3.0);
+    o.w = 0.f;
+    src[p * 8] = o;
 #pragma unroll
     for (int k = 0; k < 7; ++k) {
         double l0, l1, l2, w;
         quad7(k, l0, l1, l2, w);
-        float4 o;
-        o.x = (float)(l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0]);
-        o.y = (float)(l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]);
-        o.z = (float)(l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]);
-        o.w = (float)(sA * w);
-        src[p * 7 + k] = o;
+        float4 r;
+        r.x = (float)((l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0]) - (double)o.x);
+        r.y = (float)((l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]) - (double)o.y);
+        r.z = (float)((l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]) - (double)o.z);
+        r.w = (float)(sA * w);
+        src[p * 8 + 1 + k] = r;
     }
 }
 
@@ -422,8 +577,20 @@ __global__ void set_sigma_kernel(const float* __restrict__ sigma, const double* 
     for (int k = 0; k < 7; ++k) {
         double l0, l1, l2, w;
         quad7(k, l0, l1, l2, w);
-        src[p * 7 + k].w = (float)(sA * w);
+        src[p * 8 + 1 + k].w = (float)(sA * w);
     }
+}
+
+/* inspection: quadrature sources back in global coordinates, [np*7] float4 (x, y, z, w) */
+__global__ void unpack_panels_kernel(const float4* __restrict__ src, float4* __restrict__ out, long long np)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= np * 7) return;
+    const long long p = i / 7;
+    const int k = (int)(i - p * 7);
+    const float4 o = src[p * 8], r = src[p * 8 + 1 + k];
+    out[i] = make_float4((float)((double)o.x + (double)r.x), (float)((double)o.y + (double)r.y),
+                         (float)((double)o.z + (double)r.z), r.w);
 }
 
 /* ------------------------------------------------------------------------------------------- */
@@ -531,6 +698,7 @@ bool aligned16(const void* p) { return (((uintptr_t)p) & 15u) == 0; }
 bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
 
 long long pad_sb(long long n) { return ceil_div(n, SB) * SB; }
+long long pad_panels(long long np) { return ceil_div(np, PANELS_PER_BLOCK) * PANELS_PER_BLOCK; }
 
 int grow_charges(obem_ctx* c, long long n)
 {
@@ -550,7 +718,7 @@ int grow_panels(obem_ctx* c, long long np)
     if (need <= c->pan_cap) return OBEM_OK;
     float4* p = nullptr;
     double* a = nullptr;
-    OBEM_CUDA(c, cudaMalloc(&p, (size_t)pad_sb(need * 7) * sizeof(float4)));
+    OBEM_CUDA(c, cudaMalloc(&p, (size_t)pad_panels(need) * 8 * sizeof(float4)));
     cudaError_t e = cudaMalloc(&a, (size_t)need * sizeof(double));
     if (e != cudaSuccess) {
         cudaFree(p);
@@ -577,7 +745,7 @@ int grow_stage(obem_ctx* c, int i, size_t bytes)
 }
 
 /* the evaluation proper: targets tgt[0..nt) -> out[0..nt) */
-int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, bool at_charges,
+int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                 cudaStream_t st)
 {
     if (flags & ~(OBEM_NBODY | OBEM_PANELS)) return OBEM_EINVAL;
@@ -590,25 +758,22 @@ int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsig
     P.sec[0].src = P.sec[1].src = nullptr;
     P.sec[0].nblk = P.sec[1].nblk = 0;
     P.sec[0].eps2 = P.sec[1].eps2 = 0.f;
-    P.self_sub = 0;
-    P.self_eps2 = 0.f;
+    P.sec[0].kind = P.sec[1].kind = KIND_POINTS;
+    P.self_first = -1;
     if ((flags & OBEM_NBODY) && c->n_chg > 0) {
         P.sec[ns].src = c->d_chg;
         P.sec[ns].nblk = ceil_div(c->n_chg, SB);
         P.sec[ns].eps2 = c->eps_pp * c->eps_pp;
-        /* reading A3: the self term is excluded by index.  With softening it is the exactly known
-         * amount q_i * rsqrt(eps^2) in phi (and exactly 0 in E): the kernels subtract it.  Without
-         * softening the zero-distance guard (reading A4) already drops it. */
-        if (at_charges && P.sec[ns].eps2 > 0.f) {
-            P.self_sub = 1;
-            P.self_eps2 = P.sec[ns].eps2;
-        }
+        P.sec[ns].kind = KIND_POINTS;
+        /* reading A3: at the charges, target i IS source self_first + i and is excluded by index */
+        if (self_first >= 0) P.self_first = self_first;
         ++ns;
     }
     if ((flags & OBEM_PANELS) && c->n_pan > 0) {
         P.sec[ns].src = c->d_psrc;
-        P.sec[ns].nblk = ceil_div(c->n_pan * 7, SB);
+        P.sec[ns].nblk = ceil_div(c->n_pan, PANELS_PER_BLOCK);
         P.sec[ns].eps2 = c->eps_panel * c->eps_panel;
+        P.sec[ns].kind = KIND_PANELS;
         ++ns;
     }
     if (ns == 0) {
@@ -724,11 +889,9 @@ int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int
     int rc = grow_panels(c, n_panels);
     if (rc != OBEM_OK) return rc;
     if (n_panels > 0) {
-        const long long ns = n_panels * 7, ns_pad = pad_sb(ns);
-        if (ns_pad > ns)
-            OBEM_CUDA(c, cudaMemsetAsync(c->d_psrc + ns, 0, (size_t)(ns_pad - ns) * sizeof(float4), st));
-        pack_panels_kernel<<<(unsigned)ceil_div(n_panels, 128), 128, 0, st>>>(d_verts, d_sigma, c->d_psrc,
-                                                                              c->d_area, n_panels);
+        const long long np_pad = pad_panels(n_panels);
+        pack_panels_kernel<<<(unsigned)ceil_div(np_pad, 128), 128, 0, st>>>(d_verts, d_sigma, c->d_psrc, c->d_area,
+                                                                           n_panels, np_pad);
         OBEM_CUDA(c, cudaGetLastError());
         c->launches += 1;
     }
@@ -777,7 +940,7 @@ int obem_eval_at_charges_range(obem_ctx* c, int64_t first, int64_t count, float*
     if (first + count > c->n_chg) return OBEM_EINVAL;
     if (count > 0 && (!d_out || !aligned16(d_out))) return OBEM_EINVAL;
     DeviceGuard g(c->device);
-    return eval_common(c, c->d_chg + first, count, (float4*)d_out, flags, true, (cudaStream_t)cuda_stream);
+    return eval_common(c, c->d_chg + first, count, (float4*)d_out, flags, first, (cudaStream_t)cuda_stream);
 }
 
 int obem_eval_at_charges(obem_ctx* c, float* d_out, unsigned flags, void* cuda_stream)
@@ -792,7 +955,7 @@ int obem_eval_at_points(obem_ctx* c, const float* d_pts, int64_t m, float* d_out
     if (!c || m < 0) return OBEM_EINVAL;
     if (m > 0 && (!d_pts || !d_out || !aligned16(d_pts) || !aligned16(d_out))) return OBEM_EINVAL;
     DeviceGuard g(c->device);
-    return eval_common(c, (const float4*)d_pts, m, (float4*)d_out, flags, false, (cudaStream_t)cuda_stream);
+    return eval_common(c, (const float4*)d_pts, m, (float4*)d_out, flags, -1, (cudaStream_t)cuda_stream);
 }
 
 static int host_set_panels(obem_ctx* c, const float* h_verts, const float* h_sigma, int64_t np)
@@ -883,8 +1046,10 @@ int obem_get_panel_sources(obem_ctx* c, float* d_out, void* cuda_stream)
     if (c->n_pan == 0) return OBEM_OK;
     if (!d_out || !aligned16(d_out)) return OBEM_EINVAL;
     DeviceGuard g(c->device);
-    OBEM_CUDA(c, cudaMemcpyAsync(d_out, c->d_psrc, (size_t)c->n_pan * 7 * sizeof(float4), cudaMemcpyDeviceToDevice,
-                                 (cudaStream_t)cuda_stream));
+    unpack_panels_kernel<<<(unsigned)ceil_div(c->n_pan * 7, 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+        c->d_psrc, (float4*)d_out, c->n_pan);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
     return OBEM_OK;
 }
 
