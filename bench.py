@@ -47,7 +47,7 @@ _CLOCK_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.a
 class ClockSampler:
     """nvidia-smi sampling DURING the timed region (B200_PROFILING.md's clocks line)."""
 
-    def __init__(self, gpu_index: int):
+    def __init__(self, gpu_index):
         self.gpu = gpu_index
         self.proc = None
         self.path = None
@@ -123,3 +123,318 @@ def shard_range(n: int, world: int, rank: int):
     base, rem = divmod(n, world)
     first = rank * base + min(rank, rem)
     return first, base + (1 if rank < rem else 0)
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CPU oracle, timed as it stands (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample_rate(wl, seconds: float, seed: int = 123):
+    """Time oracle/ (fp64, OpenMP over targets, all host cores) on a bounded seeded sample of the workload's
+    targets against ALL its sources.  Returns (interactions_per_s, cores, sample_description, seconds_used)."""
+    from oracle import ref  # test infrastructure: allowed here (cpu_baseline / --impl reference only)
+    ref.build()
+    cores = ref.max_threads()
+    rng = np.random.default_rng(seed)
+    nt = wl.n_targets
+    per_target = (wl.n_charges - (1 if wl.points is None else 0)) + 7 * wl.n_panels
+    targets_all = wl.points if wl.points is not None else wl.xyzq
+
+    def run(idx):
+        tg = targets_all[idx]
+        si = idx.astype(np.int64) if wl.points is None else None
+        t0 = time.perf_counter()
+        ref.eval_field(xyzq=wl.xyzq, verts=wl.verts, sigma=wl.sigma, targets=tg, self_index=si,
+                       eps_pp=wl.eps_pp, eps_panel=wl.eps_panel)
+        return time.perf_counter() - t0
+
+    probe = np.sort(rng.choice(nt, min(nt, 4 * cores), replace=False))
+    tp = max(run(probe), 1e-6)
+    rate = len(probe) * per_target / tp
+    n_s = int(min(nt, max(len(probe), seconds * rate / per_target)))
+    idx = np.sort(rng.choice(nt, n_s, replace=False))
+    ts = run(idx)
+    rate = n_s * per_target / ts
+    desc = "%d seeded targets of %d against all %d charges + %d panels (%.3g interactions, %.1f s)" % (
+        n_s, nt, wl.n_charges, wl.n_panels, n_s * per_target, ts)
+    return rate, cores, desc, ts
+
+
+def workload_config(wl, args, world):
+    return {
+        "workload": "BASELINE.json configs[%d] '%s': %d charges (e-/ions), %d triangular panels, Plummer eps %.3g m; "
+                    "E and phi at every charge" % (wl.cfg - 1, wl.name, wl.n_charges, wl.n_panels, wl.eps_pp),
+        "n_charges": wl.n_charges, "n_panels": wl.n_panels, "n_targets": wl.n_targets,
+        "interactions_per_step": wl.interactions()["total"],
+        "step": "set_panels + set_charges + eval_at_charges(NBODY|PANELS)" +
+                (" with NCCL all-gather of the charge slices" if world > 1 else ""),
+        "sharding": "targets sharded over %d rank(s), sources replicated" % world,
+        "l2": "flushed between timed steps (%d MiB memset, outside the events)" % (L2_FLUSH_BYTES >> 20),
+        "seed": "numpy default_rng([0, %d])" % wl.cfg,
+    }
+
+
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    wl = W.make_workload(args.config)
+    total = wl.interactions()["total"]
+    per_step = max(2.0, min(args.cpu_seconds, 120.0 / max(1, args.steps + args.warmup)))
+    vals, cores, desc = [], 1, ""
+    for i in range(args.warmup + args.steps):
+        rate, cores, desc, _ = oracle_sample_rate(wl, per_step, seed=1000 + i)
+        if i >= args.warmup:
+            vals.append(rate)
+    rate = float(np.mean(vals)) if vals else 0.0
+    value = rate / 1e9
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": (total / rate * 1e3) if rate > 0 else None,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(wl, args, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "each step: " + desc + "; ms_per_step is the full workload extrapolated"},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2110_09214_b200 import build as _build
+    if rank == 0:
+        _build.build_lib()
+    if world > 1:
+        dist.barrier()
+    from paper_2110_09214_b200 import api
+
+    wl = W.make_workload(args.config)           # every rank generates the same seeded inputs
+    if wl.points is not None:
+        raise SystemExit("bench.py times evaluation at the charges (configs 1-4); config 5 is a parity case")
+    n, npan = wl.n_charges, wl.n_panels
+    first, count = shard_range(n, world, rank)
+    per_target = (n - 1) + 7 * npan
+    total_inter = n * per_target
+    my_inter = count * per_target
+
+    ctx = api.Context(local)
+    ctx.reserve(n, npan)
+    ctx.set_softening(wl.eps_pp, wl.eps_panel)
+    d_verts = torch.from_numpy(wl.verts).to(dev)
+    d_sigma = torch.from_numpy(wl.sigma).to(dev)
+    d_x = torch.from_numpy(wl.xyzq).to(dev)
+    d_slice = d_x[first:first + count].clone()
+    equal = (n % world == 0)
+    d_all = torch.empty_like(d_x)
+    out = torch.empty((count, 4), dtype=torch.float32, device=dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def gather_charges():
+        if world == 1:
+            return d_x
+        if equal:
+            dist.all_gather_into_tensor(d_all, d_slice)
+        else:
+            parts = [torch.empty((shard_range(n, world, r)[1], 4), dtype=torch.float32, device=dev)
+                     for r in range(world)]
+            dist.all_gather(parts, d_slice)
+            torch.cat(parts, out=d_all)
+        return d_all
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+
+    def step(timers=None):
+        flush.zero_()                                   # L2 flush, outside the events
+        if timers is not None:
+            timers[0].record(stream)
+        ctx.set_panels(d_verts, d_sigma)
+        ctx.set_charges(gather_charges())
+        if timers is not None:
+            timers[1].record(stream)
+        ctx.eval_at_charges_range(first, count, out=out, flags=api.NBODY | api.PANELS)
+        if timers is not None:
+            timers[2].record(stream)
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    sync_all()
+
+    uuid = getattr(torch.cuda.get_device_properties(local), "uuid", None)
+    sampler = ClockSampler("GPU-%s" % uuid if uuid else str(local))
+    if rank == 0:
+        sampler.start()
+    launches0 = ctx.kernel_launches
+    timers = [[ev(), ev(), ev()] for _ in range(args.steps)]
+    sync_all()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        step(timers[k])
+    sync_all()
+    wall = time.perf_counter() - wall0
+    launches = ctx.kernel_launches - launches0
+    clocks = sampler.stop() if rank == 0 else {}
+
+    step_ms = [t[0].elapsed_time(t[2]) for t in timers]
+    eval_ms = [t[1].elapsed_time(t[2]) for t in timers]
+    tot_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tot_ms, op=dist.ReduceOp.MAX)     # max over ranks, device-timed
+    ms_per_step = float(tot_ms.item()) / max(args.steps, 1)
+    value = total_inter / (ms_per_step * 1e-3) / 1e9
+
+    # ---- end to end through host buffers ---------------------------------------------------------
+    e2e_steps = max(1, min(args.steps, 3))
+    h_x = torch.from_numpy(wl.xyzq).pin_memory()
+    h_v = torch.from_numpy(wl.verts).pin_memory()
+    h_s = torch.from_numpy(wl.sigma).pin_memory()
+    h_out = torch.empty((count, 4), dtype=torch.float32).pin_memory()
+    h_slice = h_x[first:first + count]
+    h2d = d2h = 0
+
+    def e2e_step():
+        nonlocal h2d, d2h
+        if world == 1:
+            # ONE C-ABI call with host pointers: H2D of every input, set_panels, set_charges, eval, D2H
+            ctx.field_at_charges_host(h_x.numpy(), h_v.numpy(), h_s.numpy(), out=h_out.numpy(),
+                                      flags=api.NBODY | api.PANELS)
+            h2d = h_x.numel() * 4 + h_v.numel() * 4 + h_s.numel() * 4
+        else:
+            d_slice.copy_(h_slice, non_blocking=True)
+            d_verts.copy_(h_v, non_blocking=True)
+            d_sigma.copy_(h_s, non_blocking=True)
+            ctx.set_panels(d_verts, d_sigma)
+            ctx.set_charges(gather_charges())
+            ctx.eval_at_charges_range(first, count, out=out, flags=api.NBODY | api.PANELS)
+            h_out.copy_(out, non_blocking=True)
+            torch.cuda.synchronize()
+            h2d = h_slice.numel() * 4 + h_v.numel() * 4 + h_s.numel() * 4
+        d2h = h_out.numel() * 4
+
+    e2e_step()
+    sync_all()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    sync_all()
+    e2e_s = torch.tensor([(time.perf_counter() - t0) / e2e_steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+    e2e_value = total_inter / float(e2e_s.item()) / 1e9
+
+    # ---- supplementary, N = 1 only: N-body alone (the north_star's 60 % target) and the FP32 pipe probe ----
+    extras = {}
+    if world == 1:
+        def timed(fn, reps=3):
+            fn()
+            torch.cuda.synchronize()
+            best = 1e30
+            for _ in range(reps):
+                a, b = ev(), ev()
+                flush.zero_()
+                a.record(stream)
+                fn()
+                b.record(stream)
+                torch.cuda.synchronize()
+                best = min(best, a.elapsed_time(b) * 1e-3)
+            return best
+        t_nb = timed(lambda: ctx.eval_at_charges(out=out, flags=api.NBODY))
+        t_pn = timed(lambda: ctx.eval_at_charges(out=out, flags=api.PANELS))
+        fl = [0.0]
+
+        def probe(mode):
+            def f():
+                fl[0] = ctx.fma_peak_probe(mode, 100000)
+            t = timed(f)
+            return fl[0] / t / 1e12
+        extras = {"nbody_only": {"s": t_nb, "Ginteractions_per_s": n * (n - 1) / t_nb / 1e9},
+                  "panels_only": {"s": t_pn, "Ginteractions_per_s": 7 * npan * n / t_pn / 1e9},
+                  "fp32_probe_tflops": {"FFMA": probe(0), "FFMA2": probe(1)}}
+
+    # ---- roofline of the dominant kernel (obem_eval_kernel) -------------------------------------------
+    sm_count = ctx.sm_count
+    sm_max = (clocks.get("sm_max_mhz") or 1965.0) if rank == 0 else 1965.0
+    peak = sm_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12           # TFLOP/s
+    eval_s = float(np.mean(eval_ms)) * 1e-3
+    achieved = FLOP_PER_INTERACTION * my_inter / eval_s / 1e12
+    alg_bytes = 16 * n + 128 * npan + 16 * count + 16 * count                 # sources once, targets in, results out
+    roofline = {
+        "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+        "traffic": TRAFFIC_BYTES_PER_LAUNCH if world == 1 and args.config == 3 else None,
+        "kernel": "obem_eval_kernel (+ obem_fixup_kernel, < 0.1 % of it) between CUDA events on the launch stream",
+        "peak_source": "derived: %d SMs x %d FP32 lanes x 2 flop x clocks.max.sm %.0f MHz (DESIGN.md); "
+                       "MEASURED_PEAKS.json has no FP32 figure" % (sm_count, FP32_LANES_PER_SM, sm_max),
+        "flop_per_interaction": FLOP_PER_INTERACTION, "interactions_per_launch": my_inter,
+        "avg_launch_ms": eval_s * 1e3,
+        "algorithmic_bytes_per_launch": alg_bytes, "achieved_hbm_gbs": alg_bytes / eval_s / 1e9,
+    }
+    if extras:
+        roofline["nbody_only_frac"] = FLOP_PER_INTERACTION * extras["nbody_only"]["Ginteractions_per_s"] / 1e3 / peak
+        roofline["frac_of_measured_ffma2_peak"] = (achieved / extras["fp32_probe_tflops"]["FFMA2"]
+                                                   if extras["fp32_probe_tflops"]["FFMA2"] else None)
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rate, cores, desc, _ = oracle_sample_rate(wl, args.cpu_seconds)
+        cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": workload_config(wl, args, world),
+            "field_evals_per_s": n / (ms_per_step * 1e-3),
+            "pct_fp32_peak": 100.0 * FLOP_PER_INTERACTION * value * 1e9 / 1e12 / (peak * world),
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "api": "obem_field_at_charges_host (one C-ABI call, pinned host buffers)" if world == 1 else
+                           "per rank: pinned H2D of its slice + panels, all-gather, set_*, eval range, D2H"},
+            "gpu_launches": int(launches),
+            "roofline": roofline,
+            "cpu_baseline": cpu_baseline,
+            "wall_s_timed_region": wall,
+        }
+        line.update(extras)
+        print(json.dumps(line), flush=True)
+    ctx.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from
+# the `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None until captured.
+TRAFFIC_BYTES_PER_LAUNCH = None
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())
