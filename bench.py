@@ -32,6 +32,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 from paper_2110_09214_b200 import workloads as W  # noqa: E402  (no CUDA needed)
+from paper_2110_09214_b200.sharding import all_gather_charges, shard_range  # noqa: E402
 
 METRIC = "G pairwise interactions/s (1M-charge field eval: E and phi at every charge, N-body + panels)"
 UNIT = "Ginteractions/s"
@@ -116,13 +117,6 @@ def dist_env():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     return rank, world, local
-
-
-def shard_range(n: int, world: int, rank: int):
-    """Contiguous target slice of rank `rank`: sizes differ by at most one."""
-    base, rem = divmod(n, world)
-    first = rank * base + min(rank, rem)
-    return first, base + (1 if rank < rem else 0)
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -240,23 +234,13 @@ def run_ours(args):
     d_sigma = torch.from_numpy(wl.sigma).to(dev)
     d_x = torch.from_numpy(wl.xyzq).to(dev)
     d_slice = d_x[first:first + count].clone()
-    equal = (n % world == 0)
     d_all = torch.empty_like(d_x)
     out = torch.empty((count, 4), dtype=torch.float32, device=dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     stream = torch.cuda.current_stream()
 
     def gather_charges():
-        if world == 1:
-            return d_x
-        if equal:
-            dist.all_gather_into_tensor(d_all, d_slice)
-        else:
-            parts = [torch.empty((shard_range(n, world, r)[1], 4), dtype=torch.float32, device=dev)
-                     for r in range(world)]
-            dist.all_gather(parts, d_slice)
-            torch.cat(parts, out=d_all)
-        return d_all
+        return d_x if world == 1 else all_gather_charges(d_slice, n, out=d_all)
 
     ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
 
