@@ -158,7 +158,7 @@ __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem
 /* evaluation kernel                                                                            */
 /* ------------------------------------------------------------------------------------------- */
 struct Section {
-    const float4* src; /* packed sources, SB float4 per block (layout by kind), padded with weight-0 entries */
+    const float4* src; /* packed sources, SBH float4 per block (header + layout by kind), padded with weight-0 entries */
     long long nblk;    /* number of SB-blocks                                                            */
     float eps2;        /* softening^2 of this section                                                    */
     int kind;          /* KIND_POINTS: SB point sources (x, y, z, w) per block.
@@ -166,6 +166,12 @@ struct Section {
                           followed by 7 quadrature sources (x - c_x, y - c_y, z - c_z, w) in that frame. */
 };
 constexpr int KIND_POINTS = 0, KIND_PANELS = 1;
+/* Every source block is stored as SBH = 1 + SB float4: a header then the SB entries, so that one TMA copy
+ * brings both.  Header of a KIND_POINTS block: .x = the weight all its SB sources share, or NaN if they do
+ * not (then .y.. unused).  Identical particles (electrons, singly charged ions) make whole blocks uniform,
+ * and a uniform block needs one packed instruction less per interaction (block_loop_uniform). */
+constexpr int SBH = SB + 1;
+constexpr unsigned BLOCK_BYTES = SBH * sizeof(float4);
 constexpr int PANELS_PER_BLOCK = SB / 8;
 
 struct EvalParams {
@@ -179,7 +185,20 @@ struct EvalParams {
     float4* ws;           /* [grid][2][TT] partial sums of split tiles                                   */
     long long self_first; /* >= 0: target i IS point source (self_first + i) of sec[0] and is excluded
                              from its own sum by index (reading A3); -1: no exclusion                    */
+    unsigned* bad_count;  /* number of targets whose result came out non-finite (see obem_repair_kernel) */
+    long long* bad_list;  /* their indices, at most BAD_CAP                                               */
 };
+constexpr unsigned BAD_CAP = 1u << 20;
+
+__device__ __forceinline__ bool all_finite(float a, float b, float c, float d)
+{
+    return isfinite(a) && isfinite(b) && isfinite(c) && isfinite(d);
+}
+__device__ __forceinline__ void report_bad(const EvalParams& P, long long i)
+{
+    const unsigned k = atomicAdd(P.bad_count, 1u);
+    if (k < BAD_CAP) P.bad_list[k] = i;
+}
 
 /* first work unit of CTA c: floor(c * U / G) */
 __device__ __forceinline__ long long unit_begin(long long c, long long U, long long G)
@@ -227,8 +246,8 @@ __device__ __forceinline__ void item_back(const u64 dx, const u64 dy, const u64 
     az = fma2(sE, dz, az);
 }
 
-/* One block of SB point sources against the thread's TPT targets (KIND_POINTS). */
-template <bool GUARD>
+/* One block of SB point sources against the thread's TPT targets (KIND_POINTS).  Unguarded: see the
+ * "speculative zero-distance handling" note at obem_repair_kernel. */
 __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                            u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
@@ -247,13 +266,57 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
-                item_front<GUARD>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+                item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
                 item_back(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
             }
         }
+    }
+}
+
+/*
+ * Same for a block whose SB sources all carry the weight w (header): sum_j w f(r_j) = w sum_j f(r_j), so the
+ * weight is applied once per block and the body is 12 packed instructions: phi += u, u^2, u^3, E += u^3 d.
+ */
+__device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2, const float w,
+                                                   const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
+                                                   const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
+                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
+{
+    const u64 e2 = pk(eps2, eps2);
+    constexpr int K = UNR * NPAIR;
+#pragma unroll 1
+    for (int j0 = 0; j0 < SB; j0 += UNR) {
+        float4 q[UNR];
+#pragma unroll
+        for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j];
+        u64 dX[K], dY[K], dZ[K], U[K];
+#pragma unroll
+        for (int k = 0; k < K + DEPTH; ++k) {
+            if (k < K) {
+                const int j = k / NPAIR, p = k % NPAIR;
+                item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+            }
+            if (k >= DEPTH) {
+                const int kk = k - DEPTH, p = kk % NPAIR;
+                aP[p] = add2(aP[p], U[kk]);
+                const u64 u2 = mul2(U[kk], U[kk]);
+                const u64 u3 = mul2(u2, U[kk]);
+                aX[p] = fma2(u3, dX[kk], aX[p]);
+                aY[p] = fma2(u3, dY[kk], aY[p]);
+                aZ[p] = fma2(u3, dZ[kk], aZ[p]);
+            }
+        }
+    }
+    const u64 w2 = pk(w, w);
+#pragma unroll
+    for (int p = 0; p < NPAIR; ++p) {
+        aX[p] = mul2(aX[p], w2);
+        aY[p] = mul2(aY[p], w2);
+        aZ[p] = mul2(aZ[p], w2);
+        aP[p] = mul2(aP[p], w2);
     }
 }
 
@@ -265,7 +328,6 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
  * relative error of 1e-4..1e-2 in the field of a source 10-100 nm away; relative to the panel's own
  * centroid the same rounding is ~100x smaller, and t - c is exact for nearby targets (Sterbenz).
  */
-template <bool GUARD>
 __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                            u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
@@ -290,7 +352,7 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
-                item_front<GUARD>(dX[k], dY[k], dZ[k], U[k], TX[p], TY[p], TZ[p], q[j].x, q[j].y, q[j].z, e2);
+                item_front<false>(dX[k], dY[k], dZ[k], U[k], TX[p], TY[p], TZ[p], q[j].x, q[j].y, q[j].z, e2);
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
@@ -329,12 +391,12 @@ __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, co
 
 __device__ __forceinline__ const float4* unit_src(const EvalParams& P, long long blk)
 {
-    return (blk < P.sec[0].nblk) ? P.sec[0].src + blk * SB : P.sec[1].src + (blk - P.sec[0].nblk) * SB;
+    return (blk < P.sec[0].nblk) ? P.sec[0].src + blk * SBH : P.sec[1].src + (blk - P.sec[0].nblk) * SBH;
 }
 
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
 {
-    __shared__ __align__(128) float4 ring[STAGES][SB];
+    __shared__ __align__(128) float4 ring[STAGES][SBH];
     __shared__ __align__(8) u64 full[STAGES];
 
     const int tid = threadIdx.x;
@@ -352,8 +414,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
     long long pu = u0, pblk = u0 % P.nblk;
     if (tid == 0) {
         for (int s = 0; s < STAGES - 1 && pu < u1; ++s) {
-            mbar_expect_tx(&full[s], SB * sizeof(float4));
-            tma_load_1d(&ring[s][0], unit_src(P, pblk), SB * sizeof(float4), &full[s]);
+            mbar_expect_tx(&full[s], BLOCK_BYTES);
+            tma_load_1d(&ring[s][0], unit_src(P, pblk), BLOCK_BYTES, &full[s]);
             ++pu;
             if (++pblk == P.nblk) pblk = 0;
         }
@@ -394,8 +456,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
             if (tid == 0 && pu < u1) {
                 const int ps = (it + STAGES - 1) % STAGES;
-                mbar_expect_tx(&full[ps], SB * sizeof(float4));
-                tma_load_1d(&ring[ps][0], unit_src(P, pblk), SB * sizeof(float4), &full[ps]);
+                mbar_expect_tx(&full[ps], BLOCK_BYTES);
+                tma_load_1d(&ring[ps][0], unit_src(P, pblk), BLOCK_BYTES, &full[ps]);
                 ++pu;
                 if (++pblk == P.nblk) pblk = 0;
             }
@@ -408,18 +470,16 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             const bool first_sec = blk < P.sec[0].nblk;
             const float eps2 = first_sec ? P.sec[0].eps2 : P.sec[1].eps2;
             const int kind = first_sec ? P.sec[0].kind : P.sec[1].kind;
-            const float4* sblk = &ring[st][0];
+            const float4* sblk = &ring[st][1];
+            const float blkw = ring[st][0].x; /* header: common weight of the block, or NaN */
             if (kind == KIND_PANELS) {
-                if (eps2 > 0.0f)
-                    panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
-                else
-                    panel_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                panel_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
             } else if (first_sec && self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo) {
                 self_block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, self_lo + tid - blk * SB, THREADS);
-            } else if (eps2 > 0.0f) {
-                block_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            } else if (blkw == blkw) {
+                block_loop_uniform(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP);
             } else {
-                block_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
             }
             /* second accumulation level: flush the block sums into the running sums */
 #pragma unroll
@@ -442,8 +502,14 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             upk(RP[p], a.w, b.w);
             if (whole) {
                 const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
-                if (i0 < P.nt) P.out[i0] = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
-                if (i1 < P.nt) P.out[i1] = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
+                if (i0 < P.nt) {
+                    P.out[i0] = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
+                    if (!all_finite(a.x, a.y, a.z, a.w)) report_bad(P, i0);
+                }
+                if (i1 < P.nt) {
+                    P.out[i1] = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
+                    if (!all_finite(b.x, b.y, b.z, b.w)) report_bad(P, i1);
+                }
             } else {
                 wsl[(2 * p) * THREADS] = a;
                 wsl[(2 * p + 1) * THREADS] = b;
@@ -485,6 +551,80 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
             ph += (double)v.w;
         }
         P.out[i] = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
+        if (!(isfinite(ex) && isfinite(ey) && isfinite(ez) && isfinite(ph))) report_bad(P, i);
+    }
+}
+
+/*
+ * Speculative zero-distance handling (reading A4).  The hot loops do NOT test r2 > 0: a source at exactly
+ * zero unsoftened distance makes rsqrt return +inf and the target's sums come out inf/NaN.  That is
+ * detected when the target is written, its index is appended to bad_list, and this kernel recomputes such
+ * targets from scratch with the guard, in fp64, one CTA per target.  It costs two instructions per
+ * interaction less in the hot loop (panels: +15 %); exact coincidence of a target with a source is a
+ * measure-zero event for the path's inputs, so the list is almost always empty.  (The self term of a charge
+ * is not such an event: it is excluded by index in self_block_loop.)
+ */
+__global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P)
+{
+    __shared__ double red[4][THREADS];
+    const unsigned n = min(*P.bad_count, BAD_CAP);
+    const int tid = threadIdx.x;
+    for (unsigned r = blockIdx.x; r < n; r += gridDim.x) {
+        const long long i = P.bad_list[r];
+        const float4 t = P.tgt[i];
+        const double tx = t.x, ty = t.y, tz = t.z;
+        double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
+        for (int sct = 0; sct < 2; ++sct) {
+            const Section& S = P.sec[sct];
+            const double e2 = (double)S.eps2;
+            const long long nent = S.nblk * SB;
+            if (S.kind == KIND_POINTS) {
+                const long long self = (sct == 0 && P.self_first >= 0) ? P.self_first + i : -1;
+                for (long long j = tid; j < nent; j += THREADS) {
+                    const float4 q = S.src[(j / SB) * SBH + 1 + (j % SB)];
+                    if (j == self || q.w == 0.0f) continue;
+                    const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
+                    const double r2 = dx * dx + dy * dy + dz * dz + e2;
+                    if (!(r2 > 0.0)) continue;
+                    const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
+                    ph += w;
+                    ex += s3 * dx;
+                    ey += s3 * dy;
+                    ez += s3 * dz;
+                }
+            } else {
+                for (long long j = tid; j < nent; j += THREADS) {
+                    if ((j & 7) == 0) continue; /* frame origins */
+                    const long long e = (j / SB) * SBH + 1 + (j % SB);
+                    const float4 o = S.src[e - (j & 7)], q = S.src[e];
+                    if (q.w == 0.0f) continue;
+                    /* same arithmetic as the hot loop: shift into the frame in fp32, then subtract the offset */
+                    const double dx = (double)(t.x - o.x) - q.x, dy = (double)(t.y - o.y) - q.y,
+                                 dz = (double)(t.z - o.z) - q.z;
+                    const double r2 = dx * dx + dy * dy + dz * dz + e2;
+                    if (!(r2 > 0.0)) continue;
+                    const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
+                    ph += w;
+                    ex += s3 * dx;
+                    ey += s3 * dy;
+                    ez += s3 * dz;
+                }
+            }
+        }
+        red[0][tid] = ex;
+        red[1][tid] = ey;
+        red[2][tid] = ez;
+        red[3][tid] = ph;
+        __syncthreads();
+        for (int h = THREADS / 2; h > 0; h >>= 1) {
+            if (tid < h)
+                for (int c = 0; c < 4; ++c) red[c][tid] += red[c][tid + h];
+            __syncthreads();
+        }
+        if (tid == 0)
+            P.out[i] = make_float4((float)(KE_D * red[0][0]), (float)(KE_D * red[1][0]), (float)(KE_D * red[2][0]),
+                                   (float)(KE_D * red[3][0]));
+        __syncthreads();
     }
 }
 
@@ -493,12 +633,25 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
 /* ------------------------------------------------------------------------------------------- */
 constexpr float PAD_FAR = 1.0e15f;
 
-__global__ void pack_charges_kernel(const float4* __restrict__ in, float4* __restrict__ out, long long n,
-                                    long long n_pad)
+/* first float4 of panel p inside the blocked panel buffer (header + 32 panels x 8 float4 per block) */
+__device__ __forceinline__ long long panel_entry(long long p)
 {
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    /* padding: weight 0, parked far away so that it is never at zero distance from a target */
-    if (i < n_pad) out[i] = (i < n) ? in[i] : make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+    return (p / PANELS_PER_BLOCK) * SBH + 1 + (p % PANELS_PER_BLOCK) * 8;
+}
+
+/* One CTA of SB threads per source block: plain copy (the targets of eval_at_charges), blocked copy with
+ * header (the sources), padding (weight 0, parked far away so that it is never at zero distance from a
+ * target), and the header's common weight (NaN if the block's weights differ). */
+__global__ void __launch_bounds__(SB) pack_charges_kernel(const float4* __restrict__ in, float4* __restrict__ plain,
+                                                           float4* __restrict__ blocked, long long n)
+{
+    const long long b = blockIdx.x, i = b * SB + threadIdx.x;
+    const float4 v = (i < n) ? in[i] : make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+    if (i < n) plain[i] = v;
+    blocked[b * SBH + 1 + threadIdx.x] = v;
+    const float w0 = in[b * SB].w; /* b * SB < n for every launched block */
+    const int uniform = __syncthreads_and(v.w == w0);
+    if (threadIdx.x == 0) blocked[b * SBH] = make_float4(uniform ? w0 : __int_as_float(0x7fc00000), 0.f, 0.f, 0.f);
 }
 
 /* 7-point degree-5 triangle rule (Radon): barycentric coordinate pattern (a, b, b) and weights,
@@ -530,10 +683,12 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
 {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np_pad) return;
+    const long long e = panel_entry(p);
+    if (p % PANELS_PER_BLOCK == 0) src[e - 1] = make_float4(__int_as_float(0x7fc00000), 0.f, 0.f, 0.f); /* header */
     if (p >= np) {
-        src[p * 8] = make_float4(0.f, 0.f, 0.f, 0.f);
+        src[e] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-        for (int k = 0; k < 7; ++k) src[p * 8 + 1 + k] = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+        for (int k = 0; k < 7; ++k) src[e + 1 + k] = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
         return;
     }
     double v[3][3];
@@ -552,7 +707,7 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
     o.y = (float)((v[0][1] + v[1][1] + v[2][1]) / 3.0);
     o.z = (float)((v[0][2] + v[1][2] + v[2][2]) / 3.0);
     o.w = 0.f;
-    src[p * 8] = o;
+    src[e] = o;
 #pragma unroll
     for (int k = 0; k < 7; ++k) {
         double l0, l1, l2, w;
@@ -562,7 +717,7 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
         r.y = (float)((l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]) - (double)o.y);
         r.z = (float)((l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]) - (double)o.z);
         r.w = (float)(sA * w);
-        src[p * 8 + 1 + k] = r;
+        src[e + 1 + k] = r;
     }
 }
 
@@ -577,7 +732,7 @@ __global__ void set_sigma_kernel(const float* __restrict__ sigma, const double* 
     for (int k = 0; k < 7; ++k) {
         double l0, l1, l2, w;
         quad7(k, l0, l1, l2, w);
-        src[p * 8 + 1 + k].w = (float)(sA * w);
+        src[panel_entry(p) + 1 + k].w = (float)(sA * w);
     }
 }
 
@@ -588,7 +743,7 @@ __global__ void unpack_panels_kernel(const float4* __restrict__ src, float4* __r
     if (i >= np * 7) return;
     const long long p = i / 7;
     const int k = (int)(i - p * 7);
-    const float4 o = src[p * 8], r = src[p * 8 + 1 + k];
+    const float4 o = src[panel_entry(p)], r = src[panel_entry(p) + 1 + k];
     out[i] = make_float4((float)((double)o.x + (double)r.x), (float)((double)o.y + (double)r.y),
                          (float)((double)o.z + (double)r.z), r.w);
 }
@@ -646,8 +801,9 @@ struct obem_ctx {
     int grid = 0;
     float eps_pp = 0.f, eps_panel = 0.f;
     /* charges */
-    float4* d_chg = nullptr;
-    long long chg_cap = 0; /* capacity in float4 (padded) */
+    float4* d_chg = nullptr;     /* plain copy [n]: the targets of eval_at_charges                */
+    float4* d_chg_blk = nullptr; /* blocked copy with headers [nblk][SBH]: the sources            */
+    long long chg_cap = 0;       /* capacity in charges (a multiple of SB)                        */
     long long n_chg = -1;
     /* panels */
     float4* d_psrc = nullptr;
@@ -657,6 +813,8 @@ struct obem_ctx {
     /* split-tile workspace [grid][2][TT] */
     float4* d_ws = nullptr;
     float* d_sink = nullptr;
+    unsigned* d_bad_count = nullptr;
+    long long* d_bad_list = nullptr;
     /* staging for the *_host entry points */
     cudaStream_t hstream = nullptr;
     void* d_stage[4] = {nullptr, nullptr, nullptr, nullptr};
@@ -704,10 +862,17 @@ int grow_charges(obem_ctx* c, long long n)
 {
     const long long need = pad_sb(n > 0 ? n : 1);
     if (need <= c->chg_cap) return OBEM_OK;
-    float4* p = nullptr;
+    float4 *p = nullptr, *b = nullptr;
     OBEM_CUDA(c, cudaMalloc(&p, (size_t)need * sizeof(float4)));
+    cudaError_t e = cudaMalloc(&b, (size_t)(need / SB) * SBH * sizeof(float4));
+    if (e != cudaSuccess) {
+        cudaFree(p);
+        return cuda_fail(c, e);
+    }
     if (c->d_chg) cudaFree(c->d_chg);
+    if (c->d_chg_blk) cudaFree(c->d_chg_blk);
     c->d_chg = p;
+    c->d_chg_blk = b;
     c->chg_cap = need;
     return OBEM_OK;
 }
@@ -718,7 +883,7 @@ int grow_panels(obem_ctx* c, long long np)
     if (need <= c->pan_cap) return OBEM_OK;
     float4* p = nullptr;
     double* a = nullptr;
-    OBEM_CUDA(c, cudaMalloc(&p, (size_t)pad_panels(need) * 8 * sizeof(float4)));
+    OBEM_CUDA(c, cudaMalloc(&p, (size_t)(pad_panels(need) / PANELS_PER_BLOCK) * SBH * sizeof(float4)));
     cudaError_t e = cudaMalloc(&a, (size_t)need * sizeof(double));
     if (e != cudaSuccess) {
         cudaFree(p);
@@ -761,7 +926,7 @@ int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsig
     P.sec[0].kind = P.sec[1].kind = KIND_POINTS;
     P.self_first = -1;
     if ((flags & OBEM_NBODY) && c->n_chg > 0) {
-        P.sec[ns].src = c->d_chg;
+        P.sec[ns].src = c->d_chg_blk;
         P.sec[ns].nblk = ceil_div(c->n_chg, SB);
         P.sec[ns].eps2 = c->eps_pp * c->eps_pp;
         P.sec[ns].kind = KIND_POINTS;
@@ -787,12 +952,17 @@ int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsig
     P.U = P.ntiles * P.nblk;
     P.out = out;
     P.ws = c->d_ws;
+    P.bad_count = c->d_bad_count;
+    P.bad_list = c->d_bad_list;
+    OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
 
     obem_eval_kernel<<<c->grid, THREADS, 0, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
     obem_fixup_kernel<<<(unsigned)P.ntiles, THREADS, 0, st>>>(P, c->grid);
     OBEM_CUDA(c, cudaGetLastError());
-    c->launches += 2;
+    obem_repair_kernel<<<c->sm_count, THREADS, 0, st>>>(P);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 3;
     return OBEM_OK;
 }
 
@@ -834,6 +1004,8 @@ int obem_create(obem_ctx** out, int device)
     c->grid = c->sm_count * per_sm;
     e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_sink, 256);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_count, 256);
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_list, (size_t)BAD_CAP * sizeof(long long));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->hstream, cudaStreamNonBlocking);
     if (e != cudaSuccess) {
         int rc = cuda_fail(nullptr, e);
@@ -850,10 +1022,13 @@ int obem_destroy(obem_ctx* c)
     DeviceGuard g(c->device);
     cudaDeviceSynchronize();
     if (c->d_chg) cudaFree(c->d_chg);
+    if (c->d_chg_blk) cudaFree(c->d_chg_blk);
     if (c->d_psrc) cudaFree(c->d_psrc);
     if (c->d_area) cudaFree(c->d_area);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_sink) cudaFree(c->d_sink);
+    if (c->d_bad_count) cudaFree(c->d_bad_count);
+    if (c->d_bad_list) cudaFree(c->d_bad_list);
     for (int i = 0; i < 4; ++i)
         if (c->d_stage[i]) cudaFree(c->d_stage[i]);
     if (c->hstream) cudaStreamDestroy(c->hstream);
@@ -922,9 +1097,8 @@ int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_str
     int rc = grow_charges(c, n);
     if (rc != OBEM_OK) return rc;
     if (n > 0) {
-        const long long n_pad = pad_sb(n);
-        pack_charges_kernel<<<(unsigned)ceil_div(n_pad, 256), 256, 0, (cudaStream_t)cuda_stream>>>(
-            (const float4*)d_xyzq, c->d_chg, n, n_pad);
+        pack_charges_kernel<<<(unsigned)ceil_div(n, SB), SB, 0, (cudaStream_t)cuda_stream>>>(
+            (const float4*)d_xyzq, c->d_chg, c->d_chg_blk, n);
         OBEM_CUDA(c, cudaGetLastError());
         c->launches += 1;
     }
