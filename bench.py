@@ -409,8 +409,8 @@ def run_ours(args):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from
-# the `ncu --set full` capture summarised in profiles/ (see profiles/README.md); None until captured.
-TRAFFIC_BYTES_PER_LAUNCH = None
+# the `ncu --set full` capture summarised in profiles/r01b_summary.md: 42,320,384 B read + 2,326,016 B written.
+TRAFFIC_BYTES_PER_LAUNCH = 42320384 + 2326016
 
 
 def main():
