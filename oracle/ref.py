@@ -17,6 +17,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "obem_ref.c")
+_SRCS = [_SRC, os.path.join(_HERE, "obem_ref_next.c")]   # hot path; adjacent steps
 _LIB = os.path.join(_HERE, "libobem_ref.so")
 
 NBODY = 1
@@ -27,10 +28,10 @@ _lib = None
 
 def build(force: bool = False) -> str:
     """Compile obem_ref.c -> libobem_ref.so (gcc -O2, no fast-math, OpenMP over targets)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         tmp = _LIB + ".tmp.%d" % os.getpid()
         subprocess.check_call(
-            ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"]
+            ["gcc", "-O2", "-std=c99", "-fopenmp", "-fPIC", "-shared", "-o", tmp] + _SRCS + ["-lm"]
         )
         os.replace(tmp, _LIB)
     return _LIB
@@ -53,6 +54,14 @@ def _load():
         lib.obem_ref_quad_rule.restype = None
         lib.obem_ref_quad_rule.argtypes = [c_dp, c_dp]
         lib.obem_ref_max_threads.restype = ctypes.c_int
+        c_i32p = ctypes.POINTER(ctypes.c_int32)
+        lib.obem_ref_influence.restype = ctypes.c_int
+        lib.obem_ref_influence.argtypes = [c_fp, ctypes.c_int64, c_fp, ctypes.c_int64, ctypes.c_double,
+                                           c_dp, c_dp, c_dp, ctypes.c_int]
+        lib.obem_ref_rhs.restype = ctypes.c_int
+        lib.obem_ref_rhs.argtypes = [c_i32p, c_fp, c_fp, c_dp, c_dp, ctypes.c_int64, c_dp]
+        lib.obem_ref_matvec.restype = ctypes.c_int
+        lib.obem_ref_matvec.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, c_fp, c_dp, ctypes.c_int]
         _lib = lib
     return _lib
 
@@ -129,3 +138,53 @@ def eval_field(xyzq=None, verts=None, sigma=None, targets=None, self_index=None,
     if rc != 0:
         raise ValueError("obem_ref_eval: bad argument")
     return out_n, out_p
+
+
+# --------------------------------------------------------------------------------------------------
+# NEXT-1: influence of the particles on the cells, Eq (3.3)-(3.6); sigma = M^-1 b
+# --------------------------------------------------------------------------------------------------
+def influence(xyzq, verts, eps: float = 0.0, n_threads: int = 0):
+    """Eq (3.3)/(3.4).  Returns (infl[Np,4] = (Ebar_x, Ebar_y, Ebar_z, Vbar), en[Np] = Ebar.n, na[Np,4] = (n, A))."""
+    xyzq = _f32(xyzq if xyzq is not None else [], (4,))
+    verts = _f32(verts if verts is not None else [], (3, 3))
+    n, npan = xyzq.shape[0], verts.shape[0]
+    out = np.zeros((npan, 4), dtype=np.float64)
+    en = np.zeros(npan, dtype=np.float64)
+    na = np.zeros((npan, 4), dtype=np.float64)
+    rc = _load().obem_ref_influence(_ptr(xyzq, ctypes.c_float), n, _ptr(verts, ctypes.c_float), npan, float(eps),
+                                    _ptr(out, ctypes.c_double), _ptr(en, ctypes.c_double),
+                                    _ptr(na, ctypes.c_double), int(n_threads))
+    if rc != 0:
+        raise ValueError("obem_ref_influence: bad argument")
+    return out, en, na
+
+
+def rhs(kind, bc, deps, infl, en):
+    """Eq (3.5)/(3.6): b[Np] float64."""
+    kind = np.ascontiguousarray(kind, dtype=np.int32)
+    bc = _f32(bc, ())
+    deps = _f32(deps, ())
+    infl = np.ascontiguousarray(infl, dtype=np.float64)
+    en = np.ascontiguousarray(en, dtype=np.float64)
+    npan = kind.shape[0]
+    assert bc.shape[0] == npan and deps.shape[0] == npan and infl.shape == (npan, 4) and en.shape == (npan,)
+    b = np.zeros(npan, dtype=np.float64)
+    rc = _load().obem_ref_rhs(_ptr(kind, ctypes.c_int32), _ptr(bc, ctypes.c_float), _ptr(deps, ctypes.c_float),
+                              _ptr(infl, ctypes.c_double), _ptr(en, ctypes.c_double), npan, _ptr(b, ctypes.c_double))
+    if rc != 0:
+        raise ValueError("obem_ref_rhs: bad argument (kind must be 0 or 1)")
+    return b
+
+
+def matvec(minv, b, n_threads: int = 0):
+    """sigma = M^-1 b with a stored fp32 inverse [n, n] (row-major) and fp32 b; float64 result."""
+    minv = np.ascontiguousarray(minv, dtype=np.float32)
+    b = _f32(b, ())
+    n = b.shape[0]
+    assert minv.shape == (n, n)
+    out = np.zeros(n, dtype=np.float64)
+    rc = _load().obem_ref_matvec(_ptr(minv, ctypes.c_float), n, n, _ptr(b, ctypes.c_float),
+                                 _ptr(out, ctypes.c_double), int(n_threads))
+    if rc != 0:
+        raise ValueError("obem_ref_matvec: bad argument")
+    return out
