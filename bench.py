@@ -109,6 +109,7 @@ def parse_args():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 = the metric's workload")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the supplementary timings of the adjacent steps")
     return ap.parse_args()
 
 
@@ -356,6 +357,10 @@ def run_ours(args):
                   "panels_only": {"s": t_pn, "Ginteractions_per_s": 7 * npan * n / t_pn / 1e9},
                   "fp32_probe_tflops": {"FFMA": probe(0), "FFMA2": probe(1)}}
 
+    # ---- supplementary, N = 1 only: the adjacent steps, each against its own roofline ----
+    if world == 1 and not args.no_next:
+        extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev)
+
     # ---- roofline of the dominant kernel (obem_eval_kernel) -------------------------------------------
     sm_count = ctx.sm_count
     sm_max = (clocks.get("sm_max_mhz") or 1965.0) if rank == 0 else 1965.0
@@ -406,6 +411,54 @@ def run_ours(args):
     if world > 1:
         dist.destroy_process_group()
     return 0
+
+
+def hbm_peak_gbs():
+    """Measured HBM copy bandwidth of this pool's B200 (MEASURED_PEAKS.json, driver-written), else the fallback
+    B200_PROFILING.md states (6.65 TB/s, "of fallback")."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def bench_next1(torch, api, ctx, wl, timed, dev):
+    """Influence of the particles on the cells (Eq 3.3/3.4; FP32-pipe bound like the hot path), sigma = M^-1 b
+    (HBM bound: 4 n^2 bytes read once) and the chained dynamic update, on the bench workload."""
+    n, npan = wl.n_charges, wl.n_panels
+    peak_flops = ctx.sm_count * FP32_LANES_PER_SM * 2 * 1965.0e6 / 1e12
+    t_inf = timed(lambda: ctx.influence_on_panels())
+    inter = 7 * npan * n
+    res = {"influence": {"s": t_inf, "Ginteractions_per_s": inter / t_inf / 1e9,
+                         "frac_fp32_peak": FLOP_PER_INTERACTION * inter / t_inf / 1e12 / peak_flops,
+                         "bound": "alu"}}
+    free, _ = torch.cuda.mem_get_info()
+    ng = npan
+    while ng > 1024 and 4 * ng * ng > 0.6 * free:
+        ng //= 2
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(0)
+    minv = torch.empty((ng, ng), dtype=torch.float32, device=dev)
+    minv.normal_(0.0, 1e-10, generator=gen)
+    b = torch.randn(ng, dtype=torch.float32, device=dev, generator=gen)
+    sig = torch.empty(ng, dtype=torch.float32, device=dev)
+    t_mv = timed(lambda: ctx.apply_inverse(minv, b, out=sig), reps=5)
+    peak, src = hbm_peak_gbs()
+    gbs = 4.0 * ng * ng / t_mv / 1e9
+    res["apply_inverse"] = {"n": ng, "s": t_mv, "bound": "hbm", "achieved": gbs, "peak": peak, "unit": "GB/s",
+                            "frac": gbs / peak, "peak_source": src,
+                            "algorithmic_bytes": 4 * ng * ng + 8 * ng}
+    if ng == npan:
+        kind = (torch.arange(npan, device=dev) % 3 == 0).to(torch.int32)
+        bc = torch.zeros(npan, dtype=torch.float32, device=dev)
+        deps = torch.full((npan,), 2.5 * 8.8541878128e-12, dtype=torch.float32, device=dev)
+        sigma0 = torch.from_numpy(wl.sigma).to(dev)
+        t_dyn = timed(lambda: ctx.update_sigma_dynamic(kind, bc, deps, minv))
+        ctx.set_sigma(sigma0)
+        res["dynamic_update"] = {"s": t_dyn, "what": "influence + rhs + M^-1 b + set_sigma on one stream"}
+    del minv
+    return res
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from

@@ -137,6 +137,50 @@ int obem_get_panel_sources(obem_ctx* c, float* d_out, void* cuda_stream);
  * *flops_out (2 per scalar FMA).  Time it with events on `cuda_stream`. */
 int obem_fma_peak_probe(obem_ctx* c, int mode, int64_t iters, double* flops_out, void* cuda_stream);
 
+/* ----------------------------------------------------------------------------------------------------------
+ * Steps adjacent to the hot path: influence of the particles on the cells,
+ * PAPER.md:241-257, section 3.2.2 -- what the dynamic option does every time step BEFORE the field evaluation.
+ * ---------------------------------------------------------------------------------------------------------- */
+
+/* Eq (3.3), (3.4): area-averaged potential and field of ALL charges (obem_set_charges) over every cell C_i
+ * (obem_set_panels):
+ *     Vbar_i = k_e sum_p q_p/A_i Int_{C_i} 1/||r - r_p|| d2r,   Ebar_i = k_e sum_p q_p/A_i Int_{C_i} (r - r_p)/||r - r_p||^3 d2r
+ * with (1/A_i) Int_{C_i} f d2r = sum_k w_k f(x_ik), the same 7-point rule as the panel sums (reading A1), and the
+ * cell-particle distance softened by eps_panel (default 0 = as printed; zero distance contributes 0, reading A4).
+ *   d_infl [n_panels][4] fp32 = Ebar_x, Ebar_y, Ebar_z [V/m], Vbar [V]            (16-byte aligned)
+ *   d_en   [n_panels]    fp32 = Ebar_i . n_i, n_i = (v1-v0)x(v2-v0)/||.|| (orientation = vertex order,
+ *                               reading A16); may be NULL.
+ * OBEM_ESTATE if panels or charges were never set.  Cost: 7 * n_panels * n_charges interactions, run by the
+ * hot path's evaluation kernel, plus an O(n_panels) reduction. */
+int obem_influence_on_panels(obem_ctx* c, float* d_infl, float* d_en, void* cuda_stream);
+
+/* Eq (3.5), (3.6): the modified left-hand sides of the BEM system, per cell i:
+ *     d_kind[i] == 0 (ed cell, electrode):       b_i = V_i - Vbar_i
+ *     d_kind[i] == 1 (dd cell, dielectric face): b_i = sigma_F,i - (eps2 - eps1)_i * (Ebar_i . n_i)
+ *   d_kind [n] int32; d_bc [n] fp32 = V_i [V] or sigma_F,i [C/m^2]; d_deps [n] fp32 = eps2 - eps1 [F/m] (read for
+ *   dd cells only); d_infl [n][4], d_en [n] as written by obem_influence_on_panels; d_b [n] fp32 out.
+ * Any other kind writes NaN to b_i. */
+int obem_rhs_from_influence(obem_ctx* c, const int32_t* d_kind, const float* d_bc, const float* d_deps,
+                            const float* d_infl, const float* d_en, float* d_b, int64_t n_panels,
+                            void* cuda_stream);
+
+/* sigma = M^-1 b with the STORED inverse ("inverted once", every new right-hand side is a
+ * matrix-vector product).  d_minv [n][ld] row-major fp32 (ld >= n, caller-owned, read only), d_b [n],
+ * d_sigma [n] fp32 out.  fp32 accumulation (4 x 32 partial sums per row).  Bound by HBM: 4 n^2 bytes are read
+ * once.  The TMA-streamed kernel needs n % 4 == 0, ld % 4 == 0 and 16-byte aligned d_minv, d_b; any other shape
+ * takes a plain-load kernel (same results up to summation order). */
+int obem_apply_inverse(obem_ctx* c, const float* d_minv, int64_t n, int64_t ld, const float* d_b, float* d_sigma,
+                       void* cuda_stream);
+
+/* The dynamic-option update of one time step, enqueued on one stream:
+ * influence (3.3/3.4) -> right-hand side (3.5/3.6) -> sigma = M^-1 b -> obem_set_sigma.  d_sigma [n_panels]
+ * receives the new charge densities (and the context's panel weights are updated from it). */
+int obem_update_sigma_dynamic(obem_ctx* c, const int32_t* d_kind, const float* d_bc, const float* d_deps,
+                              const float* d_minv, int64_t ld, float* d_sigma, void* cuda_stream);
+
+/* Copy (n_x, n_y, n_z, A) of every panel to d_out [n_panels][4] fp32 -- inspection and tests. */
+int obem_get_panel_normals(obem_ctx* c, float* d_out, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

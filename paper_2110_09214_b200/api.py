@@ -44,6 +44,14 @@ SIGNATURES = {
     "obem_get_panel_sources": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
     "obem_fma_peak_probe": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, _i64, ctypes.POINTER(ctypes.c_double),
                                            ctypes.c_void_p]),
+    # adjacent steps
+    "obem_influence_on_panels": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, ctypes.c_void_p]),
+    "obem_rhs_from_influence": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _c_fp, _c_fp, _c_fp, _i64,
+                                               ctypes.c_void_p]),
+    "obem_apply_inverse": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, _i64, _c_fp, _c_fp, ctypes.c_void_p]),
+    "obem_update_sigma_dynamic": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _c_fp, _i64, _c_fp,
+                                                 ctypes.c_void_p]),
+    "obem_get_panel_normals": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
 }
 
 LIB_PATH = _build.LIB
@@ -299,3 +307,68 @@ class Context:
         self._check(_lib.obem_fma_peak_probe(self._h, int(mode), int(iters), ctypes.byref(fl), _stream_ptr(stream)),
                     "obem_fma_peak_probe")
         return fl.value
+
+    # -- adjacent steps: Eq (3.3)-(3.6), sigma = M^-1 b ---------------------------
+    def _new(self, shape):
+        torch = _torch()
+        return torch.empty(shape, dtype=torch.float32, device="cuda:%d" % self.device)
+
+    def influence_on_panels(self, want_en: bool = True, stream=None):
+        """Eq (3.3)/(3.4): returns (infl [Np,4] = Ebar_xyz, Vbar; en [Np] = Ebar.n or None)."""
+        n = max(self.n_panels, 0)
+        infl = self._new((n, 4))
+        en = self._new((n,)) if want_en else None
+        self._check(_lib.obem_influence_on_panels(self._h, infl.data_ptr() if n else None,
+                                                  en.data_ptr() if (want_en and n) else None, _stream_ptr(stream)),
+                    "obem_influence_on_panels")
+        return infl, en
+
+    def rhs_from_influence(self, kind, bc, deps, infl, en, stream=None):
+        """Eq (3.5)/(3.6): kind int32 [Np] (0 = ed, 1 = dd), bc/deps float32 [Np] -> b [Np]."""
+        torch = _torch()
+        n = int(kind.shape[0])
+        if n:
+            if not (kind.is_cuda and kind.dtype == torch.int32 and kind.is_contiguous()):
+                raise TypeError("kind must be a contiguous int32 CUDA tensor")
+            _dev_f32(bc, "bc"), _dev_f32(deps, "deps"), _dev_f32(infl, "infl", (4,)), _dev_f32(en, "en")
+        b = self._new((n,))
+        self._check(_lib.obem_rhs_from_influence(self._h, kind.data_ptr() if n else None, bc.data_ptr() if n else None,
+                                                 deps.data_ptr() if n else None, infl.data_ptr() if n else None,
+                                                 en.data_ptr() if n else None, b.data_ptr() if n else None, n,
+                                                 _stream_ptr(stream)), "obem_rhs_from_influence")
+        return b
+
+    def apply_inverse(self, minv, b, out=None, stream=None):
+        """sigma = M^-1 b: minv [n, n] (or a row-major view with stride(0) >= n), b [n] -> sigma [n]."""
+        torch = _torch()
+        n = int(b.shape[0])
+        ld = n
+        if n:
+            _dev_f32(b, "b")
+            if not (isinstance(minv, torch.Tensor) and minv.is_cuda and minv.dtype == torch.float32 and minv.dim() == 2
+                    and minv.shape == (n, n) and minv.stride(1) == 1 and minv.stride(0) >= n):
+                raise TypeError("minv must be a float32 CUDA [n, n] tensor with unit column stride")
+            ld = int(minv.stride(0))
+        if out is None:
+            out = self._new((n,))
+        self._check(_lib.obem_apply_inverse(self._h, minv.data_ptr() if n else None, n, ld, b.data_ptr() if n else None,
+                                            out.data_ptr() if n else None, _stream_ptr(stream)), "obem_apply_inverse")
+        return out
+
+    def update_sigma_dynamic(self, kind, bc, deps, minv, stream=None):
+        """influence -> rhs -> M^-1 b -> set_sigma on one stream; returns the new sigma [Np]."""
+        n = max(self.n_panels, 0)
+        sigma = self._new((n,))
+        ld = int(minv.stride(0)) if n else 0
+        self._check(_lib.obem_update_sigma_dynamic(self._h, kind.data_ptr() if n else None, bc.data_ptr() if n else None,
+                                                   deps.data_ptr() if n else None, minv.data_ptr() if n else None, ld,
+                                                   sigma.data_ptr() if n else None, _stream_ptr(stream)),
+                    "obem_update_sigma_dynamic")
+        return sigma
+
+    def get_panel_normals(self, stream=None):
+        n = max(self.n_panels, 0)
+        out = self._new((n, 4))
+        self._check(_lib.obem_get_panel_normals(self._h, out.data_ptr() if n else None, _stream_ptr(stream)),
+                    "obem_get_panel_normals")
+        return out

@@ -1,4 +1,4 @@
-"""In-tree build of libobem.so (csrc/obem.cu -> paper_2110_09214_b200/libobem.so) with nvcc for sm_100a.
+"""In-tree build of libobem.so (csrc/*.cu -> paper_2110_09214_b200/libobem.so) with nvcc for sm_100a.
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box with gpurun.
 """
@@ -11,6 +11,8 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(_HERE)
 SRC = os.path.join(_HERE, "csrc", "obem.cu")
+SRCS = [SRC, os.path.join(_HERE, "csrc", "obem_next.cu")]          # hot path; adjacent steps
+DEPS = SRCS + [os.path.join(_HERE, "csrc", "obem_internal.cuh")]
 HDR = os.path.join(ROOT, "include", "obem.h")
 LIB = os.path.join(_HERE, "libobem.so")
 
@@ -32,7 +34,7 @@ def is_stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > t for f in (SRC, HDR))
+    return any(os.path.getmtime(f) > t for f in DEPS + [HDR])
 
 
 def build_lib(force: bool = False, verbose: bool = False) -> str:
@@ -41,7 +43,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
         return LIB
     tmp = LIB + ".tmp.%d" % os.getpid()
     cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [
-        "-I", os.path.join(ROOT, "include"), "-o", tmp, SRC]
+        "-I", os.path.join(ROOT, "include"), "-o", tmp] + SRCS
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

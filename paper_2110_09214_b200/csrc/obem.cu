@@ -21,16 +21,12 @@
  *
  * This file shares no code, header, table or constant with oracle/.
  */
-#include <cuda_runtime.h>
-#include <stdint.h>
-#include <math.h>
 #include <new>
 
-#include "obem.h"
+#include "obem_internal.cuh"
 
 namespace {
 
-typedef unsigned long long u64;
 
 /* Tuning knobs (overridable with -D for sweeps; the defaults are the measured best) */
 #ifndef OBEM_THREADS
@@ -62,97 +58,6 @@ static_assert(TPT % 2 == 0 && SB % UNR == 0, "bad tuning knobs");
 
 /* k_e = 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), reading A7 */
 constexpr double KE_D = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12);
-
-/* ------------------------------------------------------------------------------------------- */
-/* packed f32x2 helpers (PTX ISA: add/sub/mul/fma .f32x2, sm_100+).  A u64 holds {lo, hi}.       */
-/* ------------------------------------------------------------------------------------------- */
-__device__ __forceinline__ u64 pk(float lo, float hi)
-{
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-/* same, but opaque to the optimiser: the pair is built once and kept (used for loop-invariant targets,
- * which the compiler would otherwise re-pack from their float4 registers inside the hot loop) */
-__device__ __forceinline__ u64 pk_keep(float lo, float hi)
-{
-    u64 r;
-    asm volatile("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void upk(u64 v, float& lo, float& hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
-{
-    u64 r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-    return r;
-}
-__device__ __forceinline__ u64 add2(u64 a, u64 b)
-{
-    u64 r;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ u64 sub2(u64 a, u64 b)
-{
-    u64 r;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ u64 mul2(u64 a, u64 b)
-{
-    u64 r;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-__device__ __forceinline__ float rsqrt_approx(float x)
-{
-    float r;
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); /* one MUFU.RSQ */
-    return r;
-}
-
-/* ------------------------------------------------------------------------------------------- */
-/* mbarrier + 1-D TMA bulk copy (global -> shared)                                              */
-/* ------------------------------------------------------------------------------------------- */
-__device__ __forceinline__ uint32_t smem_u32(const void* p)
-{
-    return (uint32_t)__cvta_generic_to_shared(p);
-}
-__device__ __forceinline__ void mbar_init(u64* bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(u64* bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(u64* bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
-        : "memory");
-}
-__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, u64* bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-            smem_u32(dst_smem)),
-        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
 
 /* ------------------------------------------------------------------------------------------- */
 /* evaluation kernel                                                                            */
@@ -678,8 +583,8 @@ __device__ __forceinline__ void quad7(int k, double& l0, double& l1, double& l2,
  * fp64 and rounded once.  Frame origin c = the centroid rounded to fp32; sources are stored as
  * (x_k - c) in fp32 (see panel_loop).  Slots >= np are padding (weight 0, parked far away). */
 __global__ void pack_panels_kernel(const float* __restrict__ verts, const float* __restrict__ sigma,
-                                   float4* __restrict__ src, double* __restrict__ area, long long np,
-                                   long long np_pad)
+                                   float4* __restrict__ src, double* __restrict__ area, float4* __restrict__ qpts,
+                                   float4* __restrict__ nrm, long long np, long long np_pad)
 {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np_pad) return;
@@ -699,8 +604,12 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
     const double ax = v[1][0] - v[0][0], ay = v[1][1] - v[0][1], az = v[1][2] - v[0][2];
     const double bx = v[2][0] - v[0][0], by = v[2][1] - v[0][1], bz = v[2][2] - v[0][2];
     const double cx = ay * bz - az * by, cy = az * bx - ax * bz, cz = ax * by - ay * bx;
-    const double A = 0.5 * sqrt(cx * cx + cy * cy + cz * cz);
+    const double clen = sqrt(cx * cx + cy * cy + cz * cz);
+    const double A = 0.5 * clen;
     area[p] = A;
+    /* unit normal (orientation = vertex order, reading A16) and area: Eq (3.6) needs Ebar . n */
+    nrm[p] = (clen > 0.0) ? make_float4((float)(cx / clen), (float)(cy / clen), (float)(cz / clen), (float)A)
+                          : make_float4(0.f, 0.f, 0.f, 0.f);
     const double sA = (double)sigma[p] * A;
     float4 o;
     o.x = (float)((v[0][0] + v[1][0] + v[2][0]) / 3.0);
@@ -718,6 +627,10 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
         r.z = (float)((l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]) - (double)o.z);
         r.w = (float)(sA * w);
         src[e + 1 + k] = r;
+        /* the same point in global coordinates with the bare rule weight: the targets of the influence pass */
+        qpts[p * 7 + k] = make_float4((float)(l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0]),
+                                      (float)(l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]),
+                                      (float)(l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]), (float)w);
     }
 }
 
@@ -788,72 +701,15 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) fma_probe_kernel(float* 
     }
 }
 
-inline long long ceil_div(long long a, long long b) { return (a + b - 1) / b; }
 
 } /* namespace */
 
 /* ------------------------------------------------------------------------------------------- */
 /* context and C ABI                                                                            */
 /* ------------------------------------------------------------------------------------------- */
-struct obem_ctx {
-    int device = 0;
-    int sm_count = 0;
-    int grid = 0;
-    float eps_pp = 0.f, eps_panel = 0.f;
-    /* charges */
-    float4* d_chg = nullptr;     /* plain copy [n]: the targets of eval_at_charges                */
-    float4* d_chg_blk = nullptr; /* blocked copy with headers [nblk][SBH]: the sources            */
-    long long chg_cap = 0;       /* capacity in charges (a multiple of SB)                        */
-    long long n_chg = -1;
-    /* panels */
-    float4* d_psrc = nullptr;
-    double* d_area = nullptr;
-    long long pan_cap = 0; /* capacity in panels */
-    long long n_pan = -1;
-    /* split-tile workspace [grid][2][TT] */
-    float4* d_ws = nullptr;
-    float* d_sink = nullptr;
-    unsigned* d_bad_count = nullptr;
-    long long* d_bad_list = nullptr;
-    /* staging for the *_host entry points */
-    cudaStream_t hstream = nullptr;
-    void* d_stage[4] = {nullptr, nullptr, nullptr, nullptr};
-    size_t stage_cap[4] = {0, 0, 0, 0};
-    long long launches = 0;
-    int last_cuda = 0;
-};
 
 namespace {
 
-struct DeviceGuard {
-    int prev = -1;
-    bool ok = true;
-    explicit DeviceGuard(int dev)
-    {
-        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
-        if (prev != dev) ok = (cudaSetDevice(dev) == cudaSuccess);
-    }
-    ~DeviceGuard()
-    {
-        if (prev >= 0) cudaSetDevice(prev);
-    }
-};
-
-int cuda_fail(obem_ctx* c, cudaError_t e)
-{
-    if (c) c->last_cuda = (int)e;
-    cudaGetLastError(); /* clear the sticky-less error state */
-    return (e == cudaErrorMemoryAllocation) ? OBEM_ENOMEM : OBEM_ECUDA;
-}
-
-#define OBEM_CUDA(c, call)                                 \
-    do {                                                   \
-        cudaError_t e__ = (call);                          \
-        if (e__ != cudaSuccess) return cuda_fail((c), e__); \
-    } while (0)
-
-bool aligned16(const void* p) { return (((uintptr_t)p) & 15u) == 0; }
-bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
 
 long long pad_sb(long long n) { return ceil_div(n, SB) * SB; }
 long long pad_panels(long long np) { return ceil_div(np, PANELS_PER_BLOCK) * PANELS_PER_BLOCK; }
@@ -881,18 +737,31 @@ int grow_panels(obem_ctx* c, long long np)
 {
     const long long need = np > 0 ? np : 1;
     if (need <= c->pan_cap) return OBEM_OK;
-    float4* p = nullptr;
+    float4 *p = nullptr, *qp = nullptr, *nr = nullptr, *it = nullptr;
     double* a = nullptr;
-    OBEM_CUDA(c, cudaMalloc(&p, (size_t)(pad_panels(need) / PANELS_PER_BLOCK) * SBH * sizeof(float4)));
-    cudaError_t e = cudaMalloc(&a, (size_t)need * sizeof(double));
+    cudaError_t e = cudaMalloc(&p, (size_t)(pad_panels(need) / PANELS_PER_BLOCK) * SBH * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&a, (size_t)need * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&qp, (size_t)need * 7 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&nr, (size_t)need * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&it, (size_t)need * 7 * sizeof(float4));
     if (e != cudaSuccess) {
-        cudaFree(p);
+        if (p) cudaFree(p);
+        if (a) cudaFree(a);
+        if (qp) cudaFree(qp);
+        if (nr) cudaFree(nr);
+        if (it) cudaFree(it);
         return cuda_fail(c, e);
     }
     if (c->d_psrc) cudaFree(c->d_psrc);
     if (c->d_area) cudaFree(c->d_area);
+    if (c->d_qpts) cudaFree(c->d_qpts);
+    if (c->d_nrm) cudaFree(c->d_nrm);
+    if (c->d_infl_tmp) cudaFree(c->d_infl_tmp);
     c->d_psrc = p;
     c->d_area = a;
+    c->d_qpts = qp;
+    c->d_nrm = nr;
+    c->d_infl_tmp = it;
     c->pan_cap = need;
     return OBEM_OK;
 }
@@ -909,9 +778,11 @@ int grow_stage(obem_ctx* c, int i, size_t bytes)
     return OBEM_OK;
 }
 
-/* the evaluation proper: targets tgt[0..nt) -> out[0..nt) */
-int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
-                cudaStream_t st)
+} /* namespace */
+
+/* the evaluation proper: targets tgt[0..nt) -> out[0..nt) (declared in obem_internal.cuh) */
+int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
+                       float eps_nbody, cudaStream_t st)
 {
     if (flags & ~(OBEM_NBODY | OBEM_PANELS)) return OBEM_EINVAL;
     if ((flags & OBEM_NBODY) && c->n_chg < 0) return OBEM_ESTATE;
@@ -928,7 +799,7 @@ int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsig
     if ((flags & OBEM_NBODY) && c->n_chg > 0) {
         P.sec[ns].src = c->d_chg_blk;
         P.sec[ns].nblk = ceil_div(c->n_chg, SB);
-        P.sec[ns].eps2 = c->eps_pp * c->eps_pp;
+        P.sec[ns].eps2 = eps_nbody * eps_nbody;
         P.sec[ns].kind = KIND_POINTS;
         /* reading A3: at the charges, target i IS source self_first + i and is excluded by index */
         if (self_first >= 0) P.self_first = self_first;
@@ -965,8 +836,6 @@ int eval_common(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsig
     c->launches += 3;
     return OBEM_OK;
 }
-
-} /* namespace */
 
 extern "C" {
 
@@ -1025,6 +894,10 @@ int obem_destroy(obem_ctx* c)
     if (c->d_chg_blk) cudaFree(c->d_chg_blk);
     if (c->d_psrc) cudaFree(c->d_psrc);
     if (c->d_area) cudaFree(c->d_area);
+    if (c->d_qpts) cudaFree(c->d_qpts);
+    if (c->d_nrm) cudaFree(c->d_nrm);
+    if (c->d_infl_tmp) cudaFree(c->d_infl_tmp);
+    if (c->d_next_scratch) cudaFree(c->d_next_scratch);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_sink) cudaFree(c->d_sink);
     if (c->d_bad_count) cudaFree(c->d_bad_count);
@@ -1066,7 +939,7 @@ int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int
     if (n_panels > 0) {
         const long long np_pad = pad_panels(n_panels);
         pack_panels_kernel<<<(unsigned)ceil_div(np_pad, 128), 128, 0, st>>>(d_verts, d_sigma, c->d_psrc, c->d_area,
-                                                                           n_panels, np_pad);
+                                                                           c->d_qpts, c->d_nrm, n_panels, np_pad);
         OBEM_CUDA(c, cudaGetLastError());
         c->launches += 1;
     }
@@ -1114,7 +987,8 @@ int obem_eval_at_charges_range(obem_ctx* c, int64_t first, int64_t count, float*
     if (first + count > c->n_chg) return OBEM_EINVAL;
     if (count > 0 && (!d_out || !aligned16(d_out))) return OBEM_EINVAL;
     DeviceGuard g(c->device);
-    return eval_common(c, c->d_chg + first, count, (float4*)d_out, flags, first, (cudaStream_t)cuda_stream);
+    return obem_eval_internal(c, c->d_chg + first, count, (float4*)d_out, flags, first, c->eps_pp,
+                              (cudaStream_t)cuda_stream);
 }
 
 int obem_eval_at_charges(obem_ctx* c, float* d_out, unsigned flags, void* cuda_stream)
@@ -1129,7 +1003,8 @@ int obem_eval_at_points(obem_ctx* c, const float* d_pts, int64_t m, float* d_out
     if (!c || m < 0) return OBEM_EINVAL;
     if (m > 0 && (!d_pts || !d_out || !aligned16(d_pts) || !aligned16(d_out))) return OBEM_EINVAL;
     DeviceGuard g(c->device);
-    return eval_common(c, (const float4*)d_pts, m, (float4*)d_out, flags, -1, (cudaStream_t)cuda_stream);
+    return obem_eval_internal(c, (const float4*)d_pts, m, (float4*)d_out, flags, -1, c->eps_pp,
+                              (cudaStream_t)cuda_stream);
 }
 
 static int host_set_panels(obem_ctx* c, const float* h_verts, const float* h_sigma, int64_t np)

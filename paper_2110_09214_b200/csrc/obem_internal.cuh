@@ -1,0 +1,190 @@
+/*
+ * obem_internal.cuh -- pieces shared by the translation units of libobem.so (obem.cu: the hot path;
+ * obem_next.cu: the adjacent steps of SURVEY.md section 8(f)).  Internal: not part of the C ABI (include/obem.h),
+ * not shared with oracle/.
+ */
+#ifndef OBEM_INTERNAL_CUH
+#define OBEM_INTERNAL_CUH
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <math.h>
+
+#include "obem.h"
+
+namespace {
+
+typedef unsigned long long u64;
+
+/* ------------------------------------------------------------------------------------------- */
+/* packed f32x2 helpers (PTX ISA: add/sub/mul/fma .f32x2, sm_100+).  A u64 holds {lo, hi}.       */
+/* ------------------------------------------------------------------------------------------- */
+__device__ __forceinline__ u64 pk(float lo, float hi)
+{
+    u64 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+/* same, but opaque to the optimiser: the pair is built once and kept (used for loop-invariant targets,
+ * which the compiler would otherwise re-pack from their float4 registers inside the hot loop) */
+__device__ __forceinline__ u64 pk_keep(float lo, float hi)
+{
+    u64 r;
+    asm volatile("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk(u64 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
+{
+    u64 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ u64 add2(u64 a, u64 b)
+{
+    u64 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 sub2(u64 a, u64 b)
+{
+    u64 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ u64 mul2(u64 a, u64 b)
+{
+    u64 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ float rsqrt_approx(float x)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); /* one MUFU.RSQ */
+    return r;
+}
+
+/* ------------------------------------------------------------------------------------------- */
+/* mbarrier + 1-D TMA bulk copy (global -> shared)                                              */
+/* ------------------------------------------------------------------------------------------- */
+__device__ __forceinline__ uint32_t smem_u32(const void* p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(u64* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(u64* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(u64* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, u64* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+            smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+
+inline long long ceil_div(long long a, long long b) { return (a + b - 1) / b; }
+
+} /* namespace */
+
+struct obem_ctx {
+    int device = 0;
+    int sm_count = 0;
+    int grid = 0;
+    float eps_pp = 0.f, eps_panel = 0.f;
+    /* charges */
+    float4* d_chg = nullptr;     /* plain copy [n]: the targets of eval_at_charges                */
+    float4* d_chg_blk = nullptr; /* blocked copy with headers [nblk][SBH]: the sources            */
+    long long chg_cap = 0;       /* capacity in charges (a multiple of SB)                        */
+    long long n_chg = -1;
+    /* panels */
+    float4* d_psrc = nullptr;
+    double* d_area = nullptr;
+    float4* d_qpts = nullptr;     /* [np*7] quadrature points in global coordinates, .w = rule weight w_k */
+    float4* d_nrm = nullptr;      /* [np] unit normal (vertex-order orientation) and area                 */
+    float4* d_infl_tmp = nullptr; /* [np*7] field of the charges at the quadrature points (influence pass) */
+    long long pan_cap = 0; /* capacity in panels */
+    long long n_pan = -1;
+    /* split-tile workspace [grid][2][TT] */
+    float4* d_ws = nullptr;
+    float* d_sink = nullptr;
+    unsigned* d_bad_count = nullptr;
+    long long* d_bad_list = nullptr;
+    /* staging for the *_host entry points */
+    cudaStream_t hstream = nullptr;
+    void* d_stage[4] = {nullptr, nullptr, nullptr, nullptr};
+    size_t stage_cap[4] = {0, 0, 0, 0};
+    long long launches = 0;
+    int last_cuda = 0;
+    /* obem_next.cu */
+    void* d_next_scratch = nullptr; /* [np][6] floats: influence, E.n and right-hand side of the dynamic update */
+    size_t next_scratch_cap = 0;
+    int gemv_attr_set = 0;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) ok = (cudaSetDevice(dev) == cudaSuccess);
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+int cuda_fail(obem_ctx* c, cudaError_t e)
+{
+    if (c) c->last_cuda = (int)e;
+    cudaGetLastError(); /* clear the sticky-less error state */
+    return (e == cudaErrorMemoryAllocation) ? OBEM_ENOMEM : OBEM_ECUDA;
+}
+
+#define OBEM_CUDA(c, call)                                 \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) return cuda_fail((c), e__); \
+    } while (0)
+
+bool aligned16(const void* p) { return (((uintptr_t)p) & 15u) == 0; }
+bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
+
+} /* namespace */
+
+/* The evaluation proper (obem.cu): targets tgt[0..nt) -> out[0..nt) on stream st.  self_first >= 0: target i IS
+ * charge self_first + i and is excluded from its own N-body sum by index.  eps_nbody: softening of the N-body
+ * section for this call (eval_at_*: eps_pp; influence on the cells: eps_panel). */
+int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
+                       float eps_nbody, cudaStream_t st);
+
+#endif /* OBEM_INTERNAL_CUH */
