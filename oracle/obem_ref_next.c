@@ -149,3 +149,49 @@ int obem_ref_matvec(const float* minv, int64_t n, int64_t ld, const float* b, do
     }
     return 0;
 }
+
+/*
+ * NEXT-2  electron-ion recombination, PAPER.md:341-355 (section 3.3.3): "taken into account microscopically for
+ * any electron and ion using the distances obtained during the N-body calculation process".  For every charge i
+ * the nearest charge of OPPOSITE sign: its true (unsoftened) distance d_i and its index j_i (ties: the smallest
+ * index; -1 and d = +infinity if there is no opposite charge).  Charges with q = 0 have no partner and are nobody's
+ * partner.
+ */
+int obem_ref_nearest_opposite(const float* xyzq, int64_t n, double* out_d, int64_t* out_j, int n_threads)
+{
+    int64_t i;
+    if (n < 0 || (n > 0 && (!xyzq || !out_d || !out_j))) return -1;
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#else
+    (void)n_threads;
+#endif
+#pragma omp parallel for schedule(dynamic, 16)
+    for (i = 0; i < n; ++i) {
+        const double x = (double)xyzq[i * 4 + 0], y = (double)xyzq[i * 4 + 1], z = (double)xyzq[i * 4 + 2];
+        const double q = (double)xyzq[i * 4 + 3];
+        double best = INFINITY;
+        int64_t bj = -1, j;
+        for (j = 0; j < n; ++j) {
+            double dx, dy, dz, r2;
+            if (j == i) continue;
+            if (!(q * (double)xyzq[j * 4 + 3] < 0.0)) continue;       /* opposite polarity only */
+            dx = x - (double)xyzq[j * 4 + 0];
+            dy = y - (double)xyzq[j * 4 + 1];
+            dz = z - (double)xyzq[j * 4 + 2];
+            r2 = dx * dx + dy * dy + dz * dz;
+            if (r2 < best) { best = r2; bj = j; }
+        }
+        out_d[i] = (bj >= 0) ? sqrt(best) : INFINITY;
+        out_j[i] = bj;
+    }
+    return 0;
+}
+
+/* Eq (3.12): a pair recombines when d <= 1/(4 pi eps0) * e / (2 E_ioni), E_ioni the ionisation
+ * energy.  With E_ioni given in eV (= volts times e) the right-hand side is k_e * e / (2 E_ioni[V]) metres. */
+double obem_ref_recombination_radius(double e_ioni_ev)
+{
+    const double e = 1.602176634e-19;
+    return next_ke() * e / (2.0 * e_ioni_ev);
+}

@@ -60,6 +60,10 @@ def _load():
                                            c_dp, c_dp, c_dp, ctypes.c_int]
         lib.obem_ref_rhs.restype = ctypes.c_int
         lib.obem_ref_rhs.argtypes = [c_i32p, c_fp, c_fp, c_dp, c_dp, ctypes.c_int64, c_dp]
+        lib.obem_ref_nearest_opposite.restype = ctypes.c_int
+        lib.obem_ref_nearest_opposite.argtypes = [c_fp, ctypes.c_int64, c_dp, c_ip, ctypes.c_int]
+        lib.obem_ref_recombination_radius.restype = ctypes.c_double
+        lib.obem_ref_recombination_radius.argtypes = [ctypes.c_double]
         lib.obem_ref_matvec.restype = ctypes.c_int
         lib.obem_ref_matvec.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, c_fp, c_dp, ctypes.c_int]
         _lib = lib
@@ -188,3 +192,24 @@ def matvec(minv, b, n_threads: int = 0):
     if rc != 0:
         raise ValueError("obem_ref_matvec: bad argument")
     return out
+
+
+# --------------------------------------------------------------------------------------------------
+# NEXT-2: recombination by-product of the N-body pass, Eq (3.12)
+# --------------------------------------------------------------------------------------------------
+def nearest_opposite(xyzq, n_threads: int = 0):
+    """(d[N] float64, j[N] int64): distance to and index of the nearest charge of opposite sign (-1 / inf if none)."""
+    xyzq = _f32(xyzq if xyzq is not None else [], (4,))
+    n = xyzq.shape[0]
+    d = np.zeros(n, dtype=np.float64)
+    j = np.zeros(n, dtype=np.int64)
+    rc = _load().obem_ref_nearest_opposite(_ptr(xyzq, ctypes.c_float), n, _ptr(d, ctypes.c_double),
+                                           _ptr(j, ctypes.c_int64), int(n_threads))
+    if rc != 0:
+        raise ValueError("obem_ref_nearest_opposite: bad argument")
+    return d, j
+
+
+def recombination_radius(e_ioni_ev: float) -> float:
+    """Eq (3.12): k_e e / (2 E_ioni) in metres, E_ioni in eV."""
+    return float(_load().obem_ref_recombination_radius(float(e_ioni_ev)))
