@@ -178,6 +178,31 @@ int obem_apply_inverse(obem_ctx* c, const float* d_minv, int64_t n, int64_t ld, 
 int obem_update_sigma_dynamic(obem_ctx* c, const int32_t* d_kind, const float* d_bc, const float* d_deps,
                               const float* d_minv, int64_t ld, float* d_sigma, void* cuda_stream);
 
+/* ----------------------------------------------------------------------------------------------------------
+ * NEXT-2: numerical integrators, section 3.2.5 -- the consumers of the field evaluation.
+ * State: d_xyzq [n][4] fp32 = x, y, z [m], q [C];  d_vel [n][4] fp32 = vx, vy, vz [m/s], m [kg] (m = 0: immobile).
+ * Non-relativistic equations of motion dx/dt = v, dv/dt = (q/m) E(x); E = the sums `flags` selects, evaluated at
+ * the charges themselves (obem_set_charges + obem_eval_at_charges on the current positions: after a step the
+ * context's charge set is the LAST positions the field was evaluated at, not the final ones).  In place, fp32.
+ * ---------------------------------------------------------------------------------------------------------- */
+
+/* x += h v (drift) and v += h (q/m) E with d_field [n][4] = Ex, Ey, Ez, phi (kick): the two sub-steps every
+ * splitting scheme is made of. */
+int obem_push_drift(obem_ctx* c, float* d_xyzq, const float* d_vel, int64_t n, float h, void* cuda_stream);
+int obem_push_kick(obem_ctx* c, const float* d_xyzq, float* d_vel, const float* d_field, int64_t n, float h,
+                   void* cuda_stream);
+
+/* Basic Euler ("a single field evaluation during a time step"):
+ *     x_{n+1} = x_n + dt v_n,   v_{n+1} = v_n + dt (q/m) E(x_n). */
+int obem_step_euler(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float dt, unsigned flags,
+                    void* cuda_stream);
+
+/* PEFRL [18] (Omelyan, Mryglod, Folk 2002: position-extended Forest-Ruth-like, 4th order, symplectic, time
+ * reversible): x v x v x v x v x with the published xi, lambda, chi -- 5 drifts, 4 kicks, i.e. 4
+ * field evaluations (reading A17: the paper counts 5). */
+int obem_step_pefrl(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float dt, unsigned flags,
+                    void* cuda_stream);
+
 /* Copy (n_x, n_y, n_z, A) of every panel to d_out [n_panels][4] fp32 -- inspection and tests. */
 int obem_get_panel_normals(obem_ctx* c, float* d_out, void* cuda_stream);
 

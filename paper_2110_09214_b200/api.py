@@ -52,6 +52,13 @@ SIGNATURES = {
     "obem_update_sigma_dynamic": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _c_fp, _i64, _c_fp,
                                                  ctypes.c_void_p]),
     "obem_get_panel_normals": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
+    # NEXT-2: integrators
+    "obem_push_drift": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_void_p]),
+    "obem_push_kick": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_void_p]),
+    "obem_step_euler": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_uint,
+                                       ctypes.c_void_p]),
+    "obem_step_pefrl": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_uint,
+                                       ctypes.c_void_p]),
 }
 
 LIB_PATH = _build.LIB
@@ -372,3 +379,35 @@ class Context:
         self._check(_lib.obem_get_panel_normals(self._h, out.data_ptr() if n else None, _stream_ptr(stream)),
                     "obem_get_panel_normals")
         return out
+
+    # -- NEXT-2: integrators; xyzq [N,4] and vel [N,4] = (vx, vy, vz, m) are updated IN PLACE ----
+    def _state(self, xyzq, vel):
+        n = int(xyzq.shape[0])
+        if n:
+            _dev_f32(xyzq, "xyzq", (4,)), _dev_f32(vel, "vel", (4,))
+            if vel.shape[0] != n:
+                raise ValueError("xyzq and vel disagree on the number of particles")
+        return n
+
+    def push_drift(self, xyzq, vel, h: float, stream=None):
+        n = self._state(xyzq, vel)
+        self._check(_lib.obem_push_drift(self._h, xyzq.data_ptr() if n else None, vel.data_ptr() if n else None, n,
+                                         float(h), _stream_ptr(stream)), "obem_push_drift")
+
+    def push_kick(self, xyzq, vel, field, h: float, stream=None):
+        n = self._state(xyzq, vel)
+        if n:
+            _dev_f32(field, "field", (4,))
+        self._check(_lib.obem_push_kick(self._h, xyzq.data_ptr() if n else None, vel.data_ptr() if n else None,
+                                        field.data_ptr() if n else None, n, float(h), _stream_ptr(stream)),
+                    "obem_push_kick")
+
+    def step_euler(self, xyzq, vel, dt: float, flags: int = NBODY | PANELS, stream=None):
+        n = self._state(xyzq, vel)
+        self._check(_lib.obem_step_euler(self._h, xyzq.data_ptr() if n else None, vel.data_ptr() if n else None, n,
+                                         float(dt), int(flags), _stream_ptr(stream)), "obem_step_euler")
+
+    def step_pefrl(self, xyzq, vel, dt: float, flags: int = NBODY | PANELS, stream=None):
+        n = self._state(xyzq, vel)
+        self._check(_lib.obem_step_pefrl(self._h, xyzq.data_ptr() if n else None, vel.data_ptr() if n else None, n,
+                                         float(dt), int(flags), _stream_ptr(stream)), "obem_step_pefrl")

@@ -63,12 +63,16 @@ constexpr double KE_D = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12);
 /* evaluation kernel                                                                            */
 /* ------------------------------------------------------------------------------------------- */
 struct Section {
-    const float4* src; /* packed sources, SBH float4 per block (header + layout by kind), padded with weight-0 entries */
-    long long nblk;    /* number of SB-blocks                                                            */
-    float eps2;        /* softening^2 of this section                                                    */
-    int kind;          /* KIND_POINTS: SB point sources (x, y, z, w) per block.
-                          KIND_PANELS: SB/8 panels per block, each 8 float4: a frame origin c (x, y, z, -)
-                          followed by 7 quadrature sources (x - c_x, y - c_y, z - c_z, w) in that frame. */
+    const float4* src;   /* packed source blocks (header + layout by kind), padded with weight-0 entries       */
+    const float4* qrel;  /* KIND_PANELS: [npan*7] plain (x - c, y - c, z - c, w_k A) of every source (repair)  */
+    long long nblk;      /* number of blocks                                                                   */
+    long long npan;      /* KIND_PANELS: number of panels                                                      */
+    int stride;          /* float4 per block: SBH (points) or SBH_P (panels)                                   */
+    float eps2;          /* softening^2 of this section                                                        */
+    int kind;            /* KIND_POINTS: header + SB point sources (x, y, z, w).
+                            KIND_PANELS: header + PPB panels of 15 float4: a frame origin c (x, y, z, -), then
+                            for each of the 7 quadrature sources the pair A = (a, b_x, b_y, b_z),
+                            B = (c_phi, a^2, w, -) of panel_encode(). */
 };
 constexpr int KIND_POINTS = 0, KIND_PANELS = 1;
 /* Every source block is stored as SBH = 1 + SB float4: a header then the SB entries, so that one TMA copy
@@ -76,8 +80,12 @@ constexpr int KIND_POINTS = 0, KIND_PANELS = 1;
  * not (then .y.. unused).  Identical particles (electrons, singly charged ions) make whole blocks uniform,
  * and a uniform block needs one packed instruction less per interaction (block_loop_uniform). */
 constexpr int SBH = SB + 1;
-constexpr unsigned BLOCK_BYTES = SBH * sizeof(float4);
-constexpr int PANELS_PER_BLOCK = SB / 8;
+/* Panel blocks: PPB panels x (1 origin + 7 x 2) float4 = 510 of 512 slots, + header. */
+constexpr int PPB = 34;
+constexpr int PANEL_SLOTS = 15;
+constexpr int SBH_P = 512 + 1;
+constexpr int RING_SLOTS = SBH_P; /* a ring stage holds the larger of the two block kinds */
+constexpr int PANELS_PER_BLOCK = PPB;
 
 struct EvalParams {
     Section sec[2];
@@ -90,6 +98,7 @@ struct EvalParams {
     float4* ws;           /* [grid][2][TT] partial sums of split tiles                                   */
     long long self_first; /* >= 0: target i IS point source (self_first + i) of sec[0] and is excluded
                              from its own sum by index (reading A3); -1: no exclusion                    */
+    int accumulate;       /* 1: add to what out already holds (the second section's launch)              */
     unsigned* bad_count;  /* number of targets whose result came out non-finite (see obem_repair_kernel) */
     long long* bad_list;  /* their indices, at most BAD_CAP                                               */
 };
@@ -226,25 +235,31 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
 }
 
 /*
- * One block of SB/8 panels (KIND_PANELS).  Each panel carries its own frame: the targets are shifted
- * into it once per panel (3 FADD2 per pair, amortised over 7 sources), and the 7 quadrature points are
- * stored relative to the frame origin.  Why: a quadrature point rounded to fp32 in GLOBAL coordinates
- * is off by up to half an ulp of the coordinate (7e-12 m at 0.2 mm, 1e-10 m at 3 mm), which is a
- * relative error of 1e-4..1e-2 in the field of a source 10-100 nm away; relative to the panel's own
- * centroid the same rounding is ~100x smaller, and t - c is exact for nearby targets (Sterbenz).
+ * One block of PPB panels (KIND_PANELS).
+ *
+ * Frames.  Each panel carries its own frame: the targets are shifted into it once per panel (3 FADD2 per pair,
+ * amortised over 7 sources), and the 7 quadrature points are stored relative to the frame origin.  Why: a
+ * quadrature point rounded to fp32 in GLOBAL coordinates is off by up to half an ulp of the coordinate (7e-12 m
+ * at 0.2 mm, 1e-10 m at 3 mm), which is a relative error of 1e-4..1e-2 in the field of a source 10-100 nm away;
+ * relative to the panel's own centroid the same rounding is ~100x smaller, and t - c is exact for nearby targets.
+ *
+ * Weight folded into the geometry (panel_encode).  For a source of weight w != 0 at offset s, with
+ * a = sign(w) / sqrt|w| and b = -a s:  d' = a (T - s) = fma(T, a, b),  r2' = d'.d' = a^2 r2,  u' = rsqrt(r2') =
+ * u / |a|, so that  u'^3 d' = w u^3 d  and  c_phi u' = w u  with c_phi = w |a|.  The weight costs no instruction:
+ * the 3 subtractions become 3 FMAs and phi's multiply-add is one FMA -- 12 packed FP32-pipe instructions per
+ * (source, target pair) instead of 13, like a uniform point block.  Softening: r2' += a^2 eps^2 (B.y = a^2).
+ * A source of weight 0 is stored as a = 0, b = 1e17: u'^3 underflows to exactly 0, c_phi = 0.
  */
+template <bool HAS_EPS>
 __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                            u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
 {
-    const u64 e2 = pk(eps2, eps2);
     constexpr int K = 7 * NPAIR;
 #pragma unroll 1
-    for (int pp = 0; pp < PANELS_PER_BLOCK; ++pp) {
-        const float4 o = s[pp * 8];
-        float4 q[7];
-#pragma unroll
-        for (int j = 0; j < 7; ++j) q[j] = s[pp * 8 + 1 + j];
+    for (int pp = 0; pp < PPB; ++pp) {
+        const float4* ps = s + pp * PANEL_SLOTS;
+        const float4 o = ps[0];
         u64 TX[NPAIR], TY[NPAIR], TZ[NPAIR];
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
@@ -252,16 +267,43 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
             TY[p] = sub2(Y[p], pk(o.y, o.y));
             TZ[p] = sub2(Z[p], pk(o.z, o.z));
         }
+        float4 qa[7];
+        float2 qb[7];
+#pragma unroll
+        for (int j = 0; j < 7; ++j) {
+            qa[j] = ps[1 + 2 * j];
+            qb[j] = *reinterpret_cast<const float2*>(ps + 2 + 2 * j);
+        }
         u64 dX[K], dY[K], dZ[K], U[K];
 #pragma unroll
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
-                item_front<false>(dX[k], dY[k], dZ[k], U[k], TX[p], TY[p], TZ[p], q[j].x, q[j].y, q[j].z, e2);
+                const u64 a2 = pk(qa[j].x, qa[j].x);
+                dX[k] = fma2(TX[p], a2, pk(qa[j].y, qa[j].y));
+                dY[k] = fma2(TY[p], a2, pk(qa[j].z, qa[j].z));
+                dZ[k] = fma2(TZ[p], a2, pk(qa[j].w, qa[j].w));
+                u64 r2;
+                if (HAS_EPS) {
+                    const float e = qb[j].y * eps2;
+                    r2 = fma2(dX[k], dX[k], pk(e, e));
+                } else {
+                    r2 = mul2(dX[k], dX[k]);
+                }
+                r2 = fma2(dY[k], dY[k], r2);
+                r2 = fma2(dZ[k], dZ[k], r2);
+                float r2l, r2h;
+                upk(r2, r2l, r2h);
+                U[k] = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
-                item_back(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
+                aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
+                const u64 u2 = mul2(U[kk], U[kk]);
+                const u64 u3 = mul2(u2, U[kk]);
+                aX[p] = fma2(u3, dX[kk], aX[p]);
+                aY[p] = fma2(u3, dY[kk], aY[p]);
+                aZ[p] = fma2(u3, dZ[kk], aZ[p]);
             }
         }
     }
@@ -296,12 +338,21 @@ __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, co
 
 __device__ __forceinline__ const float4* unit_src(const EvalParams& P, long long blk)
 {
-    return (blk < P.sec[0].nblk) ? P.sec[0].src + blk * SBH : P.sec[1].src + (blk - P.sec[0].nblk) * SBH;
+    return (blk < P.sec[0].nblk) ? P.sec[0].src + blk * P.sec[0].stride
+                                 : P.sec[1].src + (blk - P.sec[0].nblk) * P.sec[1].stride;
+}
+__device__ __forceinline__ unsigned unit_bytes(const EvalParams& P, long long blk)
+{
+    return (unsigned)((blk < P.sec[0].nblk) ? P.sec[0].stride : P.sec[1].stride) * (unsigned)sizeof(float4);
 }
 
+/* One launch per source section: KIND selects the loops compiled in (P.sec[0] is the section; P.sec[1] is empty).
+ * Two instantiations instead of one kernel with both loop families: each hot loop gets its own register
+ * allocation (a combined kernel cost the uniform N-body loop 8 extra MOVs per trip, -4 %). */
+template <int KIND>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
 {
-    __shared__ __align__(128) float4 ring[STAGES][SBH];
+    __shared__ __align__(128) float4 ring[STAGES][RING_SLOTS];
     __shared__ __align__(8) u64 full[STAGES];
 
     const int tid = threadIdx.x;
@@ -319,8 +370,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
     long long pu = u0, pblk = u0 % P.nblk;
     if (tid == 0) {
         for (int s = 0; s < STAGES - 1 && pu < u1; ++s) {
-            mbar_expect_tx(&full[s], BLOCK_BYTES);
-            tma_load_1d(&ring[s][0], unit_src(P, pblk), BLOCK_BYTES, &full[s]);
+            mbar_expect_tx(&full[s], unit_bytes(P, pblk));
+            tma_load_1d(&ring[s][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[s]);
             ++pu;
             if (++pblk == P.nblk) pblk = 0;
         }
@@ -361,8 +412,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
             if (tid == 0 && pu < u1) {
                 const int ps = (it + STAGES - 1) % STAGES;
-                mbar_expect_tx(&full[ps], BLOCK_BYTES);
-                tma_load_1d(&ring[ps][0], unit_src(P, pblk), BLOCK_BYTES, &full[ps]);
+                mbar_expect_tx(&full[ps], unit_bytes(P, pblk));
+                tma_load_1d(&ring[ps][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[ps]);
                 ++pu;
                 if (++pblk == P.nblk) pblk = 0;
             }
@@ -372,19 +423,20 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             u64 aX[NPAIR], aY[NPAIR], aZ[NPAIR], aP[NPAIR];
 #pragma unroll
             for (int p = 0; p < NPAIR; ++p) aX[p] = aY[p] = aZ[p] = aP[p] = 0ull;
-            const bool first_sec = blk < P.sec[0].nblk;
-            const float eps2 = first_sec ? P.sec[0].eps2 : P.sec[1].eps2;
-            const int kind = first_sec ? P.sec[0].kind : P.sec[1].kind;
+            const float eps2 = P.sec[0].eps2;
             const float4* sblk = &ring[st][1];
-            const float blkw = ring[st][0].x; /* header: common weight of the block, or NaN */
-            if (kind == KIND_PANELS) {
-                panel_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
-            } else if (first_sec && self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo) {
-                self_block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, self_lo + tid - blk * SB, THREADS);
-            } else if (blkw == blkw) {
-                block_loop_uniform(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP);
+            if (KIND == KIND_PANELS) {
+                if (eps2 != 0.f) panel_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                else panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
             } else {
-                block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                const float blkw = ring[st][0].x; /* header: common weight of the block, or NaN */
+                if (self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo) {
+                    self_block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, self_lo + tid - blk * SB, THREADS);
+                } else if (blkw == blkw) {
+                    block_loop_uniform(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP);
+                } else {
+                    block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                }
             }
             /* second accumulation level: flush the block sums into the running sums */
 #pragma unroll
@@ -408,12 +460,22 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             if (whole) {
                 const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
                 if (i0 < P.nt) {
-                    P.out[i0] = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
-                    if (!all_finite(a.x, a.y, a.z, a.w)) report_bad(P, i0);
+                    float4 o = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
+                    if (P.accumulate) {
+                        const float4 h = P.out[i0];
+                        o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
+                    }
+                    P.out[i0] = o;
+                    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i0);
                 }
                 if (i1 < P.nt) {
-                    P.out[i1] = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
-                    if (!all_finite(b.x, b.y, b.z, b.w)) report_bad(P, i1);
+                    float4 o = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
+                    if (P.accumulate) {
+                        const float4 h = P.out[i1];
+                        o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
+                    }
+                    P.out[i1] = o;
+                    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i1);
                 }
             } else {
                 wsl[(2 * p) * THREADS] = a;
@@ -422,6 +484,28 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
         }
         u += nrun;
     }
+}
+
+/* first float4 (the frame origin) of panel p inside the blocked panel buffer */
+__device__ __forceinline__ long long panel_entry(long long p)
+{
+    return (p / PPB) * SBH_P + 1 + (p % PPB) * PANEL_SLOTS;
+}
+
+/* The two float4 of one quadrature source (see panel_loop): weight w [C], offset (sx, sy, sz) from the frame
+ * origin, all in double; rounded once.  a is rounded first and b, c_phi are derived from the ROUNDED a, so that
+ * fma(T, a, b) = a (T - s) up to one rounding of b. */
+__device__ __forceinline__ void panel_encode(double w, double sx, double sy, double sz, float4& A, float4& B)
+{
+    if (w == 0.0 || !isfinite(w)) {
+        A = make_float4(0.f, 1.0e17f, 1.0e17f, 1.0e17f);
+        B = make_float4(0.f, 0.f, 0.f, 0.f);
+        return;
+    }
+    const float a = (float)((w > 0.0 ? 1.0 : -1.0) / sqrt(fabs(w)));
+    const double ad = (double)a;
+    A = make_float4(a, (float)(-ad * sx), (float)(-ad * sy), (float)(-ad * sz));
+    B = make_float4((float)(w * fabs(ad)), (float)(ad * ad), (float)w, 0.f);
 }
 
 /* CTA whose unit range contains unit u (ranges are [floor(cU/G), floor((c+1)U/G)) ) */
@@ -455,8 +539,13 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
             ez += (double)v.z;
             ph += (double)v.w;
         }
-        P.out[i] = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
-        if (!(isfinite(ex) && isfinite(ey) && isfinite(ez) && isfinite(ph))) report_bad(P, i);
+        float4 o = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
+        if (P.accumulate) {
+            const float4 h = P.out[i];
+            o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
+        }
+        P.out[i] = o;
+        if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i);
     }
 }
 
@@ -482,10 +571,9 @@ __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P
         for (int sct = 0; sct < 2; ++sct) {
             const Section& S = P.sec[sct];
             const double e2 = (double)S.eps2;
-            const long long nent = S.nblk * SB;
             if (S.kind == KIND_POINTS) {
                 const long long self = (sct == 0 && P.self_first >= 0) ? P.self_first + i : -1;
-                for (long long j = tid; j < nent; j += THREADS) {
+                for (long long j = tid; j < S.nblk * SB; j += THREADS) {
                     const float4 q = S.src[(j / SB) * SBH + 1 + (j % SB)];
                     if (j == self || q.w == 0.0f) continue;
                     const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
@@ -498,18 +586,20 @@ __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P
                     ez += s3 * dz;
                 }
             } else {
-                for (long long j = tid; j < nent; j += THREADS) {
-                    if ((j & 7) == 0) continue; /* frame origins */
-                    const long long e = (j / SB) * SBH + 1 + (j % SB);
-                    const float4 o = S.src[e - (j & 7)], q = S.src[e];
-                    if (q.w == 0.0f) continue;
-                    /* same arithmetic as the hot loop: shift into the frame in fp32, then subtract the offset */
+                for (long long j = tid; j < S.npan * 7; j += THREADS) {
+                    const long long pnl = j / 7;
+                    const int k = (int)(j - pnl * 7);
+                    const long long e = panel_entry(pnl);
+                    const float4 o = S.src[e], q = S.qrel[j];
+                    const float w = S.src[e + 2 + 2 * k].z;
+                    if (w == 0.0f) continue;
+                    /* shift into the frame in fp32 like the hot loop, then subtract the plain offset */
                     const double dx = (double)(t.x - o.x) - q.x, dy = (double)(t.y - o.y) - q.y,
                                  dz = (double)(t.z - o.z) - q.z;
                     const double r2 = dx * dx + dy * dy + dz * dz + e2;
                     if (!(r2 > 0.0)) continue;
-                    const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
-                    ph += w;
+                    const double u = rsqrt(r2), wu = (double)w * u, s3 = wu * u * u;
+                    ph += wu;
                     ex += s3 * dx;
                     ey += s3 * dy;
                     ez += s3 * dz;
@@ -538,11 +628,6 @@ __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P
 /* ------------------------------------------------------------------------------------------- */
 constexpr float PAD_FAR = 1.0e15f;
 
-/* first float4 of panel p inside the blocked panel buffer (header + 32 panels x 8 float4 per block) */
-__device__ __forceinline__ long long panel_entry(long long p)
-{
-    return (p / PANELS_PER_BLOCK) * SBH + 1 + (p % PANELS_PER_BLOCK) * 8;
-}
 
 /* One CTA of SB threads per source block: plain copy (the targets of eval_at_charges), blocked copy with
  * header (the sources), padding (weight 0, parked far away so that it is never at zero distance from a
@@ -579,21 +664,25 @@ __device__ __forceinline__ void quad7(int k, double& l0, double& l1, double& l2,
     l2 = (j == 2) ? a : b;
 }
 
-/* one thread per panel slot (np_pad of them): area, frame origin and the 7 quadrature sources, derived in
- * fp64 and rounded once.  Frame origin c = the centroid rounded to fp32; sources are stored as
- * (x_k - c) in fp32 (see panel_loop).  Slots >= np are padding (weight 0, parked far away). */
+/* one thread per panel slot (np_pad of them): area, normal, frame origin and the 7 quadrature sources, derived in
+ * fp64 and rounded once.  Frame origin c = the centroid rounded to fp32; sources are encoded relative to it
+ * (panel_encode; panel_loop says why).  Slots >= np are padding (weight 0). */
 __global__ void pack_panels_kernel(const float* __restrict__ verts, const float* __restrict__ sigma,
                                    float4* __restrict__ src, double* __restrict__ area, float4* __restrict__ qpts,
-                                   float4* __restrict__ nrm, long long np, long long np_pad)
+                                   float4* __restrict__ nrm, float4* __restrict__ qrel, long long np, long long np_pad)
 {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np_pad) return;
     const long long e = panel_entry(p);
-    if (p % PANELS_PER_BLOCK == 0) src[e - 1] = make_float4(__int_as_float(0x7fc00000), 0.f, 0.f, 0.f); /* header */
+    if (p % PPB == 0) {
+        src[e - 1] = make_float4(__int_as_float(0x7fc00000), 0.f, 0.f, 0.f); /* header */
+        src[e - 1 + SBH_P - 2] = make_float4(0.f, 0.f, 0.f, 0.f);            /* the two unused slots */
+        src[e - 1 + SBH_P - 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
     if (p >= np) {
         src[e] = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-        for (int k = 0; k < 7; ++k) src[e + 1 + k] = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+        for (int k = 0; k < 7; ++k) panel_encode(0.0, 0.0, 0.0, 0.0, src[e + 1 + 2 * k], src[e + 2 + 2 * k]);
         return;
     }
     double v[3][3];
@@ -610,7 +699,7 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
     /* unit normal (orientation = vertex order, reading A16) and area: Eq (3.6) needs Ebar . n */
     nrm[p] = (clen > 0.0) ? make_float4((float)(cx / clen), (float)(cy / clen), (float)(cz / clen), (float)A)
                           : make_float4(0.f, 0.f, 0.f, 0.f);
-    const double sA = (double)sigma[p] * A;
+    const double sg = (double)sigma[p];
     float4 o;
     o.x = (float)((v[0][0] + v[1][0] + v[2][0]) / 3.0);
     o.y = (float)((v[0][1] + v[1][1] + v[2][1]) / 3.0);
@@ -621,44 +710,47 @@ __global__ void pack_panels_kernel(const float* __restrict__ verts, const float*
     for (int k = 0; k < 7; ++k) {
         double l0, l1, l2, w;
         quad7(k, l0, l1, l2, w);
-        float4 r;
-        r.x = (float)((l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0]) - (double)o.x);
-        r.y = (float)((l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]) - (double)o.y);
-        r.z = (float)((l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]) - (double)o.z);
-        r.w = (float)(sA * w);
-        src[e + 1 + k] = r;
+        const double gx = l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0];
+        const double gy = l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1];
+        const double gz = l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2];
+        /* the offset is rounded to fp32 FIRST (it is what set_sigma re-encodes from), then encoded */
+        const float4 r = make_float4((float)(gx - (double)o.x), (float)(gy - (double)o.y), (float)(gz - (double)o.z),
+                                     (float)(A * w));
+        qrel[p * 7 + k] = r;
+        panel_encode(sg * A * w, (double)r.x, (double)r.y, (double)r.z, src[e + 1 + 2 * k], src[e + 2 + 2 * k]);
         /* the same point in global coordinates with the bare rule weight: the targets of the influence pass */
-        qpts[p * 7 + k] = make_float4((float)(l0 * v[0][0] + l1 * v[1][0] + l2 * v[2][0]),
-                                      (float)(l0 * v[0][1] + l1 * v[1][1] + l2 * v[2][1]),
-                                      (float)(l0 * v[0][2] + l1 * v[1][2] + l2 * v[2][2]), (float)w);
+        qpts[p * 7 + k] = make_float4((float)gx, (float)gy, (float)gz, (float)w);
     }
 }
 
-/* new sigma on the same geometry: rewrite the weights only */
+/* new sigma on the same geometry: re-encode the 7 sources of every panel from the stored offsets */
 __global__ void set_sigma_kernel(const float* __restrict__ sigma, const double* __restrict__ area,
-                                 float4* __restrict__ src, long long np)
+                                 const float4* __restrict__ qrel, float4* __restrict__ src, long long np)
 {
     const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= np) return;
     const double sA = (double)sigma[p] * area[p];
+    const long long e = panel_entry(p);
 #pragma unroll
     for (int k = 0; k < 7; ++k) {
         double l0, l1, l2, w;
         quad7(k, l0, l1, l2, w);
-        src[panel_entry(p) + 1 + k].w = (float)(sA * w);
+        const float4 r = qrel[p * 7 + k];
+        panel_encode(sA * w, (double)r.x, (double)r.y, (double)r.z, src[e + 1 + 2 * k], src[e + 2 + 2 * k]);
     }
 }
 
 /* inspection: quadrature sources back in global coordinates, [np*7] float4 (x, y, z, w) */
-__global__ void unpack_panels_kernel(const float4* __restrict__ src, float4* __restrict__ out, long long np)
+__global__ void unpack_panels_kernel(const float4* __restrict__ src, const float4* __restrict__ qrel,
+                                     float4* __restrict__ out, long long np)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= np * 7) return;
     const long long p = i / 7;
     const int k = (int)(i - p * 7);
-    const float4 o = src[panel_entry(p)], r = src[panel_entry(p) + 1 + k];
+    const float4 o = src[panel_entry(p)], r = qrel[i];
     out[i] = make_float4((float)((double)o.x + (double)r.x), (float)((double)o.y + (double)r.y),
-                         (float)((double)o.z + (double)r.z), r.w);
+                         (float)((double)o.z + (double)r.z), src[panel_entry(p) + 2 + 2 * k].z);
 }
 
 /* ------------------------------------------------------------------------------------------- */
@@ -737,19 +829,21 @@ int grow_panels(obem_ctx* c, long long np)
 {
     const long long need = np > 0 ? np : 1;
     if (need <= c->pan_cap) return OBEM_OK;
-    float4 *p = nullptr, *qp = nullptr, *nr = nullptr, *it = nullptr;
+    float4 *p = nullptr, *qp = nullptr, *nr = nullptr, *it = nullptr, *qr = nullptr;
     double* a = nullptr;
-    cudaError_t e = cudaMalloc(&p, (size_t)(pad_panels(need) / PANELS_PER_BLOCK) * SBH * sizeof(float4));
+    cudaError_t e = cudaMalloc(&p, (size_t)(pad_panels(need) / PPB) * SBH_P * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&a, (size_t)need * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&qp, (size_t)need * 7 * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&nr, (size_t)need * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&it, (size_t)need * 7 * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&qr, (size_t)need * 7 * sizeof(float4));
     if (e != cudaSuccess) {
         if (p) cudaFree(p);
         if (a) cudaFree(a);
         if (qp) cudaFree(qp);
         if (nr) cudaFree(nr);
         if (it) cudaFree(it);
+        if (qr) cudaFree(qr);
         return cuda_fail(c, e);
     }
     if (c->d_psrc) cudaFree(c->d_psrc);
@@ -757,6 +851,8 @@ int grow_panels(obem_ctx* c, long long np)
     if (c->d_qpts) cudaFree(c->d_qpts);
     if (c->d_nrm) cudaFree(c->d_nrm);
     if (c->d_infl_tmp) cudaFree(c->d_infl_tmp);
+    if (c->d_qrel) cudaFree(c->d_qrel);
+    c->d_qrel = qr;
     c->d_psrc = p;
     c->d_area = a;
     c->d_qpts = qp;
@@ -795,6 +891,9 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     P.sec[0].nblk = P.sec[1].nblk = 0;
     P.sec[0].eps2 = P.sec[1].eps2 = 0.f;
     P.sec[0].kind = P.sec[1].kind = KIND_POINTS;
+    P.sec[0].qrel = P.sec[1].qrel = nullptr;
+    P.sec[0].npan = P.sec[1].npan = 0;
+    P.sec[0].stride = P.sec[1].stride = SBH;
     P.self_first = -1;
     if ((flags & OBEM_NBODY) && c->n_chg > 0) {
         P.sec[ns].src = c->d_chg_blk;
@@ -807,7 +906,10 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     }
     if ((flags & OBEM_PANELS) && c->n_pan > 0) {
         P.sec[ns].src = c->d_psrc;
-        P.sec[ns].nblk = ceil_div(c->n_pan, PANELS_PER_BLOCK);
+        P.sec[ns].nblk = ceil_div(c->n_pan, PPB);
+        P.sec[ns].stride = SBH_P;
+        P.sec[ns].qrel = c->d_qrel;
+        P.sec[ns].npan = c->n_pan;
         P.sec[ns].eps2 = c->eps_panel * c->eps_panel;
         P.sec[ns].kind = KIND_PANELS;
         ++ns;
@@ -825,15 +927,32 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     P.ws = c->d_ws;
     P.bad_count = c->d_bad_count;
     P.bad_list = c->d_bad_list;
+    P.accumulate = 0;
     OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
 
-    obem_eval_kernel<<<c->grid, THREADS, 0, st>>>(P);
-    OBEM_CUDA(c, cudaGetLastError());
-    obem_fixup_kernel<<<(unsigned)P.ntiles, THREADS, 0, st>>>(P, c->grid);
-    OBEM_CUDA(c, cudaGetLastError());
+    /* one stream-K launch (+ fix-up) per section; the second adds to the first's result */
+    for (int k = 0; k < ns; ++k) {
+        EvalParams Q = P;
+        Q.sec[0] = P.sec[k];
+        Q.sec[1].src = nullptr;
+        Q.sec[1].nblk = 0;
+        Q.nblk = Q.sec[0].nblk;
+        Q.U = Q.ntiles * Q.nblk;
+        Q.accumulate = (k > 0);
+        if (Q.sec[0].kind == KIND_PANELS) {
+            Q.self_first = -1;
+            obem_eval_kernel<KIND_PANELS><<<c->grid, THREADS, 0, st>>>(Q);
+        } else {
+            obem_eval_kernel<KIND_POINTS><<<c->grid, THREADS, 0, st>>>(Q);
+        }
+        OBEM_CUDA(c, cudaGetLastError());
+        obem_fixup_kernel<<<(unsigned)Q.ntiles, THREADS, 0, st>>>(Q, c->grid);
+        OBEM_CUDA(c, cudaGetLastError());
+        c->launches += 2;
+    }
     obem_repair_kernel<<<c->sm_count, THREADS, 0, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
-    c->launches += 3;
+    c->launches += 1;
     return OBEM_OK;
 }
 
@@ -862,7 +981,7 @@ int obem_create(obem_ctx** out, int device)
     }
     c->sm_count = prop.multiProcessorCount;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel, THREADS, 0);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<KIND_POINTS>, THREADS, 0);
     if (e != cudaSuccess || per_sm < 1) {
         /* no sm_100a code for this device, or the kernel cannot be resident */
         cudaGetLastError();
@@ -897,7 +1016,9 @@ int obem_destroy(obem_ctx* c)
     if (c->d_qpts) cudaFree(c->d_qpts);
     if (c->d_nrm) cudaFree(c->d_nrm);
     if (c->d_infl_tmp) cudaFree(c->d_infl_tmp);
+    if (c->d_qrel) cudaFree(c->d_qrel);
     if (c->d_next_scratch) cudaFree(c->d_next_scratch);
+    if (c->d_step_field) cudaFree(c->d_step_field);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_sink) cudaFree(c->d_sink);
     if (c->d_bad_count) cudaFree(c->d_bad_count);
@@ -939,7 +1060,7 @@ int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int
     if (n_panels > 0) {
         const long long np_pad = pad_panels(n_panels);
         pack_panels_kernel<<<(unsigned)ceil_div(np_pad, 128), 128, 0, st>>>(d_verts, d_sigma, c->d_psrc, c->d_area,
-                                                                           c->d_qpts, c->d_nrm, n_panels, np_pad);
+                                                                           c->d_qpts, c->d_nrm, c->d_qrel, n_panels, np_pad);
         OBEM_CUDA(c, cudaGetLastError());
         c->launches += 1;
     }
@@ -956,7 +1077,7 @@ int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cu
     if (n_panels == 0) return OBEM_OK;
     DeviceGuard g(c->device);
     set_sigma_kernel<<<(unsigned)ceil_div(n_panels, 128), 128, 0, (cudaStream_t)cuda_stream>>>(
-        d_sigma, c->d_area, c->d_psrc, n_panels);
+        d_sigma, c->d_area, c->d_qrel, c->d_psrc, n_panels);
     OBEM_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return OBEM_OK;
@@ -1096,7 +1217,7 @@ int obem_get_panel_sources(obem_ctx* c, float* d_out, void* cuda_stream)
     if (!d_out || !aligned16(d_out)) return OBEM_EINVAL;
     DeviceGuard g(c->device);
     unpack_panels_kernel<<<(unsigned)ceil_div(c->n_pan * 7, 256), 256, 0, (cudaStream_t)cuda_stream>>>(
-        c->d_psrc, (float4*)d_out, c->n_pan);
+        c->d_psrc, c->d_qrel, (float4*)d_out, c->n_pan);
     OBEM_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return OBEM_OK;

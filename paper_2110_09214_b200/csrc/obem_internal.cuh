@@ -126,6 +126,7 @@ struct obem_ctx {
     float4* d_psrc = nullptr;
     double* d_area = nullptr;
     float4* d_qpts = nullptr;     /* [np*7] quadrature points in global coordinates, .w = rule weight w_k */
+    float4* d_qrel = nullptr;     /* [np*7] quadrature offsets from the panel's frame origin, .w = w_k A      */
     float4* d_nrm = nullptr;      /* [np] unit normal (vertex-order orientation) and area                 */
     float4* d_infl_tmp = nullptr; /* [np*7] field of the charges at the quadrature points (influence pass) */
     long long pan_cap = 0; /* capacity in panels */
@@ -145,6 +146,8 @@ struct obem_ctx {
     void* d_next_scratch = nullptr; /* [np][6] floats: influence, E.n and right-hand side of the dynamic update */
     size_t next_scratch_cap = 0;
     int gemv_attr_set = 0;
+    float4* d_step_field = nullptr; /* [n] E, phi at the charges: scratch of the steppers */
+    long long step_field_cap = 0;
 };
 
 namespace {

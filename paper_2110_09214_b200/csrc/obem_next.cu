@@ -188,6 +188,89 @@ __global__ void __launch_bounds__(256) gemv_plain_kernel(const float* __restrict
     }
 }
 
+/* ------------------------------------------------------------------------------------------- */
+/* NEXT-2: numerical integrators, PAPER.md:300-306 (section 3.2.5)                              */
+/* ------------------------------------------------------------------------------------------- */
+/* state: xyzq [n] = (x, y, z [m], q [C]), vel [n] = (vx, vy, vz [m/s], m [kg]); dx/dt = v, dv/dt = (q/m) E(x).
+ * m = 0 marks an immobile charge (q/m taken as 0). */
+__device__ __forceinline__ float q_over_m(float q, float m) { return (m != 0.f) ? q / m : 0.f; }
+
+/* drift: x += h v */
+__global__ void drift_kernel(float4* __restrict__ xyzq, const float4* __restrict__ vel, float h, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 x = xyzq[i];
+    const float4 v = vel[i];
+    x.x = fmaf(h, v.x, x.x);
+    x.y = fmaf(h, v.y, x.y);
+    x.z = fmaf(h, v.z, x.z);
+    xyzq[i] = x;
+}
+
+/* kick: v += h (q/m) E */
+__global__ void kick_kernel(const float4* __restrict__ xyzq, float4* __restrict__ vel, const float4* __restrict__ field,
+                            float h, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 v = vel[i];
+    const float4 e = field[i];
+    const float a = h * q_over_m(xyzq[i].w, v.w);
+    v.x = fmaf(a, e.x, v.x);
+    v.y = fmaf(a, e.y, v.y);
+    v.z = fmaf(a, e.z, v.z);
+    vel[i] = v;
+}
+
+/* basic Euler: x_{n+1} = x_n + h v_n, v_{n+1} = v_n + h (q/m) E(x_n) -- both from the state at the start */
+__global__ void euler_kernel(float4* __restrict__ xyzq, float4* __restrict__ vel, const float4* __restrict__ field,
+                             float h, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 x = xyzq[i];
+    float4 v = vel[i];
+    const float4 e = field[i];
+    x.x = fmaf(h, v.x, x.x);
+    x.y = fmaf(h, v.y, x.y);
+    x.z = fmaf(h, v.z, x.z);
+    const float a = h * q_over_m(x.w, v.w);
+    v.x = fmaf(a, e.x, v.x);
+    v.y = fmaf(a, e.y, v.y);
+    v.z = fmaf(a, e.z, v.z);
+    xyzq[i] = x;
+    vel[i] = v;
+}
+
+int grow_step_field(obem_ctx* c, long long n)
+{
+    if (n <= c->step_field_cap) return OBEM_OK;
+    float4* p = nullptr;
+    OBEM_CUDA(c, cudaMalloc(&p, (size_t)n * sizeof(float4)));
+    if (c->d_step_field) cudaFree(c->d_step_field);
+    c->d_step_field = p;
+    c->step_field_cap = n;
+    return OBEM_OK;
+}
+
+/* field at the current positions: set_charges(x) + eval_at_charges -> c->d_step_field */
+int field_at_state(obem_ctx* c, const float* d_xyzq, long long n, unsigned flags, void* stream)
+{
+    int rc = obem_set_charges(c, d_xyzq, n, stream);
+    if (rc != OBEM_OK) return rc;
+    return obem_eval_at_charges(c, (float*)c->d_step_field, flags, stream);
+}
+
+int step_args_ok(obem_ctx* c, const float* d_xyzq, const float* d_vel, int64_t n, unsigned flags)
+{
+    if (!c || n < 0) return OBEM_EINVAL;
+    if (flags & ~(OBEM_NBODY | OBEM_PANELS)) return OBEM_EINVAL;
+    if (n > 0 && (!d_xyzq || !d_vel || !aligned16(d_xyzq) || !aligned16(d_vel))) return OBEM_EINVAL;
+    if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
+    return OBEM_OK;
+}
+
 int grow_scratch(obem_ctx* c, long long np)
 {
     const size_t need = (size_t)(np > 0 ? np : 1) * 6 * sizeof(float);
@@ -289,6 +372,75 @@ int obem_update_sigma_dynamic(obem_ctx* c, const int32_t* d_kind, const float* d
     if (rc == OBEM_OK) rc = obem_apply_inverse(c, d_minv, np, ld, b, d_sigma, cuda_stream);
     if (rc == OBEM_OK) rc = obem_set_sigma(c, d_sigma, np, cuda_stream);
     return rc;
+}
+
+int obem_push_drift(obem_ctx* c, float* d_xyzq, const float* d_vel, int64_t n, float h, void* cuda_stream)
+{
+    if (!c || n < 0 || !isfinite(h)) return OBEM_EINVAL;
+    if (n == 0) return OBEM_OK;
+    if (!d_xyzq || !d_vel || !aligned16(d_xyzq) || !aligned16(d_vel)) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    drift_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>((float4*)d_xyzq,
+                                                                                    (const float4*)d_vel, h, n);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return OBEM_OK;
+}
+
+int obem_push_kick(obem_ctx* c, const float* d_xyzq, float* d_vel, const float* d_field, int64_t n, float h,
+                   void* cuda_stream)
+{
+    if (!c || n < 0 || !isfinite(h)) return OBEM_EINVAL;
+    if (n == 0) return OBEM_OK;
+    if (!d_xyzq || !d_vel || !d_field || !aligned16(d_xyzq) || !aligned16(d_vel) || !aligned16(d_field))
+        return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    kick_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+        (const float4*)d_xyzq, (float4*)d_vel, (const float4*)d_field, h, n);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return OBEM_OK;
+}
+
+int obem_step_euler(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float dt, unsigned flags, void* cuda_stream)
+{
+    int rc = step_args_ok(c, d_xyzq, d_vel, n, flags);
+    if (rc != OBEM_OK || !isfinite(dt)) return rc != OBEM_OK ? rc : OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    rc = grow_step_field(c, n);
+    if (rc != OBEM_OK) return rc;
+    rc = field_at_state(c, d_xyzq, n, flags, cuda_stream);
+    if (rc != OBEM_OK || n == 0) return rc;
+    euler_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+        (float4*)d_xyzq, (float4*)d_vel, c->d_step_field, dt, n);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return OBEM_OK;
+}
+
+int obem_step_pefrl(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float dt, unsigned flags, void* cuda_stream)
+{
+    int rc = step_args_ok(c, d_xyzq, d_vel, n, flags);
+    if (rc != OBEM_OK || !isfinite(dt)) return rc != OBEM_OK ? rc : OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    rc = grow_step_field(c, n);
+    if (rc != OBEM_OK) return rc;
+    /* Omelyan, Mryglod, Folk, Comput. Phys. Commun. 146 (2002) 188: position-extended Forest-Ruth-like scheme */
+    const double xi = 0.1786178958448091, lam = -0.2123418310626054, chi = -0.6626458266981849e-1;
+    const double h = (double)dt;
+    const float drift[5] = {(float)(xi * h), (float)(chi * h), (float)((1.0 - 2.0 * (chi + xi)) * h), (float)(chi * h),
+                            (float)(xi * h)};
+    const float kick[4] = {(float)((1.0 - 2.0 * lam) * 0.5 * h), (float)(lam * h), (float)(lam * h),
+                           (float)((1.0 - 2.0 * lam) * 0.5 * h)};
+    for (int s = 0; s < 5; ++s) {
+        rc = obem_push_drift(c, d_xyzq, d_vel, n, drift[s], cuda_stream);
+        if (rc != OBEM_OK) return rc;
+        if (s == 4) break;
+        rc = field_at_state(c, d_xyzq, n, flags, cuda_stream);
+        if (rc == OBEM_OK) rc = obem_push_kick(c, d_xyzq, d_vel, (const float*)c->d_step_field, n, kick[s], cuda_stream);
+        if (rc != OBEM_OK) return rc;
+    }
+    return OBEM_OK;
 }
 
 int obem_get_panel_normals(obem_ctx* c, float* d_out, void* cuda_stream)
