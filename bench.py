@@ -360,6 +360,7 @@ def run_ours(args):
     # ---- supplementary, N = 1 only: the adjacent steps, each against its own roofline ----
     if world == 1 and not args.no_next:
         extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev)
+        extras["next2"] = bench_next2(torch, api, ctx, wl, timed, dev, extras["nbody_only"]["s"])
 
     # ---- roofline of the dominant kernel (obem_eval_kernel) -------------------------------------------
     sm_count = ctx.sm_count
@@ -458,6 +459,27 @@ def bench_next1(torch, api, ctx, wl, timed, dev):
         ctx.set_sigma(sigma0)
         res["dynamic_update"] = {"s": t_dyn, "what": "influence + rhs + M^-1 b + set_sigma on one stream"}
     del minv
+    return res
+
+
+def bench_next2(torch, api, ctx, wl, timed, dev, t_nbody):
+    """Recombination by-product of the N-body pass and one Euler / PEFRL step on the
+    bench workload, N-body + panels."""
+    n = wl.n_charges
+    peak_flops = ctx.sm_count * FP32_LANES_PER_SM * 2 * 1965.0e6 / 1e12
+    t_trk = timed(lambda: ctx.eval_at_charges_partners(flags=api.NBODY))
+    res = {"nbody_with_partners": {"s": t_trk, "Ginteractions_per_s": n * (n - 1) / t_trk / 1e9,
+                                   "frac_fp32_peak": FLOP_PER_INTERACTION * n * (n - 1) / t_trk / 1e12 / peak_flops,
+                                   "overhead_vs_nbody_only": t_trk / t_nbody - 1.0}}
+    x = torch.from_numpy(wl.xyzq).to(dev)
+    v = torch.zeros_like(x)
+    v[:, 3] = 9.1093837015e-31
+    per_eval = n * ((n - 1) + 7 * wl.n_panels)
+    t_e = timed(lambda: ctx.step_euler(x, v, 25e-15), reps=2)
+    res["step_euler"] = {"s": t_e, "field_evaluations": 1, "Ginteractions_per_s": per_eval / t_e / 1e9}
+    t_p = timed(lambda: ctx.step_pefrl(x, v, 25e-15), reps=1)
+    res["step_pefrl"] = {"s": t_p, "field_evaluations": 4, "Ginteractions_per_s": 4 * per_eval / t_p / 1e9}
+    ctx.set_charges(torch.from_numpy(wl.xyzq).to(dev))
     return res
 
 

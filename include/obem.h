@@ -203,6 +203,26 @@ int obem_step_euler(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float d
 int obem_step_pefrl(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float dt, unsigned flags,
                     void* cuda_stream);
 
+/* Electron-ion recombination, PAPER.md:341-355 (section 3.3.3): "taken into account microscopically for any
+ * electron and ion using the distances obtained during the N-body calculation process".  Same as
+ * obem_eval_at_charges[_range] (flags must include OBEM_NBODY), and as a by-product of the N-body pass, for every
+ * charge i of the range, its nearest charge of OPPOSITE sign:
+ *   d_partner_d [count] fp32 = true (unsoftened) distance [m], +inf if there is none
+ *   d_partner_j [count] int32 = index of that charge in the charge set, -1 if there is none
+ * Charges with q = 0 have no partner and are nobody's partner.  How: the evaluation kernel keeps, per target, the
+ * smallest SOFTENED fp32 r2 over opposite-sign sources and the 256-source block it fell in (2 FMNMX per packed
+ * interaction on the ALU pipe); a second O(256 N) kernel scans that block exactly.  Near-ties between different
+ * blocks are decided on the fp32 softened r2: the reported distance d obeys d^2 <= d_true^2 + 4 ulp(d_true^2 +
+ * eps_pp^2).  A pair recombines when d <= obem_recombination_radius(E_ioni), Eq (3.12). */
+int obem_eval_at_charges_partners(obem_ctx* c, float* d_out, float* d_partner_d, int32_t* d_partner_j,
+                                  unsigned flags, void* cuda_stream);
+int obem_eval_at_charges_partners_range(obem_ctx* c, int64_t first, int64_t count, float* d_out,
+                                        float* d_partner_d, int32_t* d_partner_j, unsigned flags,
+                                        void* cuda_stream);
+
+/* Eq (3.12): 1/(4 pi eps0) * e / (2 E_ioni) in metres for E_ioni in eV (host arithmetic). */
+double obem_recombination_radius(double e_ioni_ev);
+
 /* Copy (n_x, n_y, n_z, A) of every panel to d_out [n_panels][4] fp32 -- inspection and tests. */
 int obem_get_panel_normals(obem_ctx* c, float* d_out, void* cuda_stream);
 

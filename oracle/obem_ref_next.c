@@ -157,17 +157,29 @@ int obem_ref_matvec(const float* minv, int64_t n, int64_t ld, const float* b, do
  * index; -1 and d = +infinity if there is no opposite charge).  Charges with q = 0 have no partner and are nobody's
  * partner.
  */
+int obem_ref_nearest_opposite_subset(const float* xyzq, int64_t n, const int64_t* idx, int64_t nidx, double* out_d,
+                                     int64_t* out_j, int n_threads);
+
 int obem_ref_nearest_opposite(const float* xyzq, int64_t n, double* out_d, int64_t* out_j, int n_threads)
 {
-    int64_t i;
-    if (n < 0 || (n > 0 && (!xyzq || !out_d || !out_j))) return -1;
+    return obem_ref_nearest_opposite_subset(xyzq, n, NULL, n, out_d, out_j, n_threads);
+}
+
+/* Same for the charges idx[0..nidx) only (idx == NULL: charge t itself, nidx = n); out_d, out_j have nidx entries.
+ * The candidates are always ALL n charges. */
+int obem_ref_nearest_opposite_subset(const float* xyzq, int64_t n, const int64_t* idx, int64_t nidx, double* out_d,
+                                     int64_t* out_j, int n_threads)
+{
+    int64_t t;
+    if (n < 0 || nidx < 0 || (nidx > 0 && (!xyzq || !out_d || !out_j))) return -1;
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
 #else
     (void)n_threads;
 #endif
 #pragma omp parallel for schedule(dynamic, 16)
-    for (i = 0; i < n; ++i) {
+    for (t = 0; t < nidx; ++t) {
+        const int64_t i = idx ? idx[t] : t;
         const double x = (double)xyzq[i * 4 + 0], y = (double)xyzq[i * 4 + 1], z = (double)xyzq[i * 4 + 2];
         const double q = (double)xyzq[i * 4 + 3];
         double best = INFINITY;
@@ -182,8 +194,8 @@ int obem_ref_nearest_opposite(const float* xyzq, int64_t n, double* out_d, int64
             r2 = dx * dx + dy * dy + dz * dz;
             if (r2 < best) { best = r2; bj = j; }
         }
-        out_d[i] = (bj >= 0) ? sqrt(best) : INFINITY;
-        out_j[i] = bj;
+        out_d[t] = (bj >= 0) ? sqrt(best) : INFINITY;
+        out_j[t] = bj;
     }
     return 0;
 }

@@ -62,6 +62,9 @@ def _load():
         lib.obem_ref_rhs.argtypes = [c_i32p, c_fp, c_fp, c_dp, c_dp, ctypes.c_int64, c_dp]
         lib.obem_ref_nearest_opposite.restype = ctypes.c_int
         lib.obem_ref_nearest_opposite.argtypes = [c_fp, ctypes.c_int64, c_dp, c_ip, ctypes.c_int]
+        lib.obem_ref_nearest_opposite_subset.restype = ctypes.c_int
+        lib.obem_ref_nearest_opposite_subset.argtypes = [c_fp, ctypes.c_int64, c_ip, ctypes.c_int64, c_dp, c_ip,
+                                                         ctypes.c_int]
         lib.obem_ref_recombination_radius.restype = ctypes.c_double
         lib.obem_ref_recombination_radius.argtypes = [ctypes.c_double]
         lib.obem_ref_matvec.restype = ctypes.c_int
@@ -197,14 +200,20 @@ def matvec(minv, b, n_threads: int = 0):
 # --------------------------------------------------------------------------------------------------
 # NEXT-2: recombination by-product of the N-body pass, Eq (3.12)
 # --------------------------------------------------------------------------------------------------
-def nearest_opposite(xyzq, n_threads: int = 0):
-    """(d[N] float64, j[N] int64): distance to and index of the nearest charge of opposite sign (-1 / inf if none)."""
+def nearest_opposite(xyzq, idx=None, n_threads: int = 0):
+    """(d, j): distance to and index of the nearest charge of opposite sign (-1 / inf if none), for every charge
+    or for the charges idx only (candidates are always all charges)."""
     xyzq = _f32(xyzq if xyzq is not None else [], (4,))
     n = xyzq.shape[0]
-    d = np.zeros(n, dtype=np.float64)
-    j = np.zeros(n, dtype=np.int64)
-    rc = _load().obem_ref_nearest_opposite(_ptr(xyzq, ctypes.c_float), n, _ptr(d, ctypes.c_double),
-                                           _ptr(j, ctypes.c_int64), int(n_threads))
+    if idx is not None:
+        idx = np.ascontiguousarray(idx, dtype=np.int64)
+        assert idx.ndim == 1 and (idx.size == 0 or (idx.min() >= 0 and idx.max() < n))
+    m = n if idx is None else idx.shape[0]
+    d = np.zeros(m, dtype=np.float64)
+    j = np.zeros(m, dtype=np.int64)
+    rc = _load().obem_ref_nearest_opposite_subset(_ptr(xyzq, ctypes.c_float), n,
+                                                  _ptr(idx, ctypes.c_int64) if idx is not None else None, m,
+                                                  _ptr(d, ctypes.c_double), _ptr(j, ctypes.c_int64), int(n_threads))
     if rc != 0:
         raise ValueError("obem_ref_nearest_opposite: bad argument")
     return d, j

@@ -52,6 +52,12 @@ SIGNATURES = {
     "obem_update_sigma_dynamic": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _c_fp, _i64, _c_fp,
                                                  ctypes.c_void_p]),
     "obem_get_panel_normals": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
+    # NEXT-2: recombination by-product of the N-body pass
+    "obem_eval_at_charges_partners": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, ctypes.c_uint,
+                                                     ctypes.c_void_p]),
+    "obem_eval_at_charges_partners_range": (ctypes.c_int, [ctypes.c_void_p, _i64, _i64, _c_fp, _c_fp, _c_fp,
+                                                           ctypes.c_uint, ctypes.c_void_p]),
+    "obem_recombination_radius": (ctypes.c_double, [ctypes.c_double]),
     # NEXT-2: integrators
     "obem_push_drift": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_void_p]),
     "obem_push_kick": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_void_p]),
@@ -411,3 +417,27 @@ class Context:
         n = self._state(xyzq, vel)
         self._check(_lib.obem_step_pefrl(self._h, xyzq.data_ptr() if n else None, vel.data_ptr() if n else None, n,
                                          float(dt), int(flags), _stream_ptr(stream)), "obem_step_pefrl")
+
+    # -- NEXT-2: recombination by-product ---------------------------------------------
+    def eval_at_charges_partners(self, flags: int = NBODY | PANELS, first: int = 0, count=None, stream=None):
+        """Returns (out [count,4], partner_d [count] float32, partner_j [count] int32) for charges [first, first+count)."""
+        torch = _torch()
+        n = self.n_charges
+        if n < 0:
+            self._check(-2, "obem_eval_at_charges_partners")
+        if count is None:
+            count = n - first
+        dev = "cuda:%d" % self.device
+        out = torch.empty((max(count, 0), 4), dtype=torch.float32, device=dev)
+        pd = torch.empty((max(count, 0),), dtype=torch.float32, device=dev)
+        pj = torch.empty((max(count, 0),), dtype=torch.int32, device=dev)
+        ok = count > 0
+        self._check(_lib.obem_eval_at_charges_partners_range(
+            self._h, int(first), int(count), out.data_ptr() if ok else None, pd.data_ptr() if ok else None,
+            pj.data_ptr() if ok else None, int(flags), _stream_ptr(stream)), "obem_eval_at_charges_partners_range")
+        return out, pd, pj
+
+
+def recombination_radius(e_ioni_ev: float) -> float:
+    """Eq (3.12): k_e e / (2 E_ioni) [m], E_ioni in eV."""
+    return float(_lib.obem_recombination_radius(float(e_ioni_ev)))

@@ -98,6 +98,8 @@ struct EvalParams {
     float4* ws;           /* [grid][2][TT] partial sums of split tiles                                   */
     long long self_first; /* >= 0: target i IS point source (self_first + i) of sec[0] and is excluded
                              from its own sum by index (reading A3); -1: no exclusion                    */
+    float2* trk_out;      /* TRACK: [nt] (min softened r2 over opposite-sign sources, its block index as int bits) */
+    float2* trk_ws;       /* TRACK: [grid][2][TT] the same for split tiles                                  */
     int accumulate;       /* 1: add to what out already holds (the second section's launch)              */
     unsigned* bad_count;  /* number of targets whose result came out non-finite (see obem_repair_kernel) */
     long long* bad_list;  /* their indices, at most BAD_CAP                                               */
@@ -128,9 +130,21 @@ __device__ __forceinline__ long long unit_begin(long long c, long long U, long l
  * GUARD (eps = 0 only): a source at zero distance contributes 0 (reading A4).
  */
 template <bool GUARD>
+__device__ __forceinline__ void item_front_r2(u64& dx, u64& dy, u64& dz, u64& u, float& r2l, float& r2h,
+                                              const u64 tx, const u64 ty, const u64 tz, const float sx,
+                                              const float sy, const float sz, const u64 e2);
+template <bool GUARD>
 __device__ __forceinline__ void item_front(u64& dx, u64& dy, u64& dz, u64& u, const u64 tx, const u64 ty,
                                            const u64 tz, const float sx, const float sy, const float sz,
                                            const u64 e2)
+{
+    float r2l, r2h;
+    item_front_r2<GUARD>(dx, dy, dz, u, r2l, r2h, tx, ty, tz, sx, sy, sz, e2);
+}
+template <bool GUARD>
+__device__ __forceinline__ void item_front_r2(u64& dx, u64& dy, u64& dz, u64& u, float& r2l, float& r2h,
+                                              const u64 tx, const u64 ty, const u64 tz, const float sx,
+                                              const float sy, const float sz, const u64 e2)
 {
     dx = sub2(tx, pk(sx, sx));
     dy = sub2(ty, pk(sy, sy));
@@ -138,7 +152,6 @@ __device__ __forceinline__ void item_front(u64& dx, u64& dy, u64& dz, u64& u, co
     u64 r2 = fma2(dx, dx, e2);
     r2 = fma2(dy, dy, r2);
     r2 = fma2(dz, dz, r2);
-    float r2l, r2h;
     upk(r2, r2l, r2h);
     float ul = rsqrt_approx(r2l);
     float uh = rsqrt_approx(r2h);
@@ -194,10 +207,11 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
  * Same for a block whose SB sources all carry the weight w (header): sum_j w f(r_j) = w sum_j f(r_j), so the
  * weight is applied once per block and the body is 12 packed instructions: phi += u, u^2, u^3, E += u^3 d.
  */
+template <bool TRACK>
 __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2, const float w,
                                                    const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
-                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
+                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
 {
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR;
@@ -211,7 +225,17 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
-                item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+                if (TRACK) {
+                    /* by-product: smallest softened r2 of the block per target, 2 FMNMX on the
+                     * otherwise idle ALU pipe; whether the block's sign is opposite is decided after the block */
+                    float r2l, r2h;
+                    item_front_r2<false>(dX[k], dY[k], dZ[k], U[k], r2l, r2h, X[p], Y[p], Z[p], q[j].x, q[j].y,
+                                         q[j].z, e2);
+                    bm[2 * p] = fminf(bm[2 * p], r2l);
+                    bm[2 * p + 1] = fminf(bm[2 * p + 1], r2h);
+                } else {
+                    item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+                }
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, p = kk % NPAIR;
@@ -316,10 +340,12 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
  * source index of the block); always guarded (d = 0 there).  Simple loop: it runs for TT/SB of the
  * blocks of a tile only.
  */
+template <bool TRACK>
 __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                              const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                              u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR],
-                                             const long long selfrel0, const int selfrel_stride)
+                                             const long long selfrel0, const int selfrel_stride, float (&bm)[TPT],
+                                             const unsigned negmask, const unsigned posmask)
 {
     const u64 e2 = pk(eps2, eps2);
 #pragma unroll 1
@@ -328,7 +354,17 @@ __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, co
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
             u64 dx, dy, dz, u;
-            item_front<true>(dx, dy, dz, u, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+            if (TRACK) {
+                /* TRACK also sends every non-uniform block here: the sign is tested per source.  The self term has
+                 * the target's own sign, so it is never a partner. */
+                const unsigned el = (q.w > 0.f) ? negmask : ((q.w < 0.f) ? posmask : 0u);
+                float r2l, r2h;
+                item_front_r2<true>(dx, dy, dz, u, r2l, r2h, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+                if ((el >> (2 * p)) & 1u) bm[2 * p] = fminf(bm[2 * p], r2l);
+                if ((el >> (2 * p + 1)) & 1u) bm[2 * p + 1] = fminf(bm[2 * p + 1], r2h);
+            } else {
+                item_front<true>(dx, dy, dz, u, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+            }
             const float wl = (selfrel0 + (long long)(2 * p) * selfrel_stride == j) ? 0.0f : q.w;
             const float wh = (selfrel0 + (long long)(2 * p + 1) * selfrel_stride == j) ? 0.0f : q.w;
             item_back(dx, dy, dz, u, pk(wl, wh), aX[p], aY[p], aZ[p], aP[p]);
@@ -349,11 +385,14 @@ __device__ __forceinline__ unsigned unit_bytes(const EvalParams& P, long long bl
 /* One launch per source section: KIND selects the loops compiled in (P.sec[0] is the section; P.sec[1] is empty).
  * Two instantiations instead of one kernel with both loop families: each hot loop gets its own register
  * allocation (a combined kernel cost the uniform N-body loop 8 extra MOVs per trip, -4 %). */
-template <int KIND>
+template <int KIND, bool TRACK>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
 {
-    __shared__ __align__(128) float4 ring[STAGES][RING_SLOTS];
+    __shared__ __align__(128) float4 ring[STAGES][KIND == KIND_PANELS ? SBH_P : SBH + 3]; /* stage stride % 64 B == 0 */
     __shared__ __align__(8) u64 full[STAGES];
+    /* TRACK: running (min r2, block) per target slot, updated once per block */
+    __shared__ float trk_m[TRACK ? TPT : 1][THREADS];
+    __shared__ int trk_b[TRACK ? TPT : 1][THREADS];
 
     const int tid = threadIdx.x;
     const long long G = gridDim.x, c = blockIdx.x;
@@ -403,6 +442,18 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
         u64 RX[NPAIR], RY[NPAIR], RZ[NPAIR], RP[NPAIR];
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) RX[p] = RY[p] = RZ[p] = RP[p] = 0ull;
+        unsigned negmask = 0u, posmask = 0u; /* TRACK: bit k set = target slot k is negative / positive */
+        if (TRACK) {
+#pragma unroll
+            for (int k = 0; k < TPT; ++k) {
+                const long long i = tbase + (long long)k * THREADS;
+                const float q = (i < P.nt) ? __ldg((const float*)(P.tgt + i) + 3) : 0.f;
+                negmask |= (q < 0.f) ? (1u << k) : 0u;
+                posmask |= (q > 0.f) ? (1u << k) : 0u;
+                trk_m[k][tid] = __int_as_float(0x7f800000);
+                trk_b[k][tid] = -1;
+            }
+        }
 
         /* source-index range of this tile's own targets inside sec[0] (evaluation at the charges) */
         const long long self_lo = (P.self_first >= 0) ? P.self_first + tile * (long long)TT : -1;
@@ -430,12 +481,30 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
                 else panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
             } else {
                 const float blkw = ring[st][0].x; /* header: common weight of the block, or NaN */
-                if (self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo) {
-                    self_block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, self_lo + tid - blk * SB, THREADS);
+                float bm[TPT];
+                unsigned elig = 0xffu; /* TRACK: target slots for which bm counts (the slow loop masks per source) */
+                if (TRACK) {
+#pragma unroll
+                    for (int k = 0; k < TPT; ++k) bm[k] = __int_as_float(0x7f800000);
+                }
+                const bool diag = self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo;
+                if (diag || (TRACK && !(blkw == blkw))) {
+                    self_block_loop<TRACK>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP,
+                                           diag ? self_lo + tid - blk * SB : -(1LL << 40), THREADS, bm, negmask, posmask);
                 } else if (blkw == blkw) {
-                    block_loop_uniform(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP);
+                    block_loop_uniform<TRACK>(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP, bm);
+                    elig = (blkw > 0.f) ? negmask : ((blkw < 0.f) ? posmask : 0u);
                 } else {
                     block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+                }
+                if (TRACK) {
+#pragma unroll
+                    for (int k = 0; k < TPT; ++k) {
+                        if (((elig >> k) & 1u) && bm[k] < trk_m[k][tid]) {
+                            trk_m[k][tid] = bm[k];
+                            trk_b[k][tid] = (int)blk;
+                        }
+                    }
                 }
             }
             /* second accumulation level: flush the block sums into the running sums */
@@ -480,6 +549,19 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             } else {
                 wsl[(2 * p) * THREADS] = a;
                 wsl[(2 * p + 1) * THREADS] = b;
+            }
+        }
+        if (TRACK) {
+            float2* tw = P.trk_ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT + tid;
+#pragma unroll
+            for (int k = 0; k < TPT; ++k) {
+                const float2 v = make_float2(trk_m[k][tid], __int_as_float(trk_b[k][tid]));
+                const long long i = tbase + (long long)k * THREADS;
+                if (whole) {
+                    if (i < P.nt) P.trk_out[i] = v;
+                } else {
+                    tw[k * THREADS] = v;
+                }
             }
         }
         u += nrun;
@@ -529,10 +611,19 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
         const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
         if (i >= P.nt) continue;
         double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
+        float tm = __int_as_float(0x7f800000);
+        int tb = -1;
         for (long long c = cA; c <= cB; ++c) {
             const long long c0 = unit_begin(c, P.U, G), c1 = unit_begin(c + 1, P.U, G);
             if (c0 >= c1) continue;
             const int slot = (c0 / P.nblk == tile) ? 0 : 1;
+            if (P.trk_out) { /* CTAs in ascending block order: strict < keeps the lowest block on ties */
+                const float2 t = P.trk_ws[((size_t)c * 2 + slot) * TT + (size_t)k * THREADS + tid];
+                if (t.x < tm) {
+                    tm = t.x;
+                    tb = __float_as_int(t.y);
+                }
+            }
             const float4 v = P.ws[((size_t)c * 2 + slot) * TT + (size_t)k * THREADS + tid];
             ex += (double)v.x;
             ey += (double)v.y;
@@ -546,6 +637,56 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
         }
         P.out[i] = o;
         if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i);
+        if (P.trk_out) P.trk_out[i] = make_float2(tm, __int_as_float(tb));
+    }
+}
+
+/*
+ * Recombination by-product, second step: the evaluation kernel left, per charge, the source
+ * block that holds its nearest opposite-sign partner (decided on the softened fp32 r2).  One warp per charge
+ * scans that block's 256 sources with exact arithmetic (fp32 coordinates promoted to double, NO softening) and
+ * writes the partner's true distance and index; ties go to the smallest index.  No opposite charge: inf, -1.
+ */
+__global__ void __launch_bounds__(256) partner_resolve_kernel(const float4* __restrict__ chg, const float4* __restrict__ blk,
+                                                              const float2* __restrict__ trk, long long first,
+                                                              long long count, long long n, float* __restrict__ out_d,
+                                                              int* __restrict__ out_j)
+{
+    const int lane = threadIdx.x & 31;
+    const long long w = (long long)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (w >= count) return;
+    const long long i = first + w;
+    const float4 t = chg[i];
+    const int b = __float_as_int(trk[w].y);
+    double best = 1.0e300;
+    int bj = 0x7fffffff;
+    if (b >= 0) {
+        const float4* src = blk + (long long)b * SBH + 1;
+        for (int k = lane; k < SB; k += 32) {
+            const long long j = (long long)b * SB + k;
+            const float4 q = src[k];
+            if (j >= n || j == i || !(q.w * t.w < 0.f)) continue;
+            const double dx = (double)t.x - (double)q.x, dy = (double)t.y - (double)q.y, dz = (double)t.z - (double)q.z;
+            const double d2 = dx * dx + dy * dy + dz * dz;
+            if (d2 < best) { /* ascending k per lane: the first (smallest) index wins ties */
+                best = d2;
+                bj = (int)j;
+            }
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double ob = __shfl_xor_sync(0xffffffffu, best, o);
+        const int oj = __shfl_xor_sync(0xffffffffu, bj, o);
+        if (ob < best || (ob == best && oj < bj)) {
+            best = ob;
+            bj = oj;
+        }
+    }
+    if (lane == 0) {
+        const bool found = bj != 0x7fffffff;
+        out_d[w] = found ? (float)sqrt(best) : __int_as_float(0x7f800000);
+        out_j[w] = found ? bj : -1;
     }
 }
 
@@ -811,16 +952,21 @@ int grow_charges(obem_ctx* c, long long n)
     const long long need = pad_sb(n > 0 ? n : 1);
     if (need <= c->chg_cap) return OBEM_OK;
     float4 *p = nullptr, *b = nullptr;
+    float2* t = nullptr;
     OBEM_CUDA(c, cudaMalloc(&p, (size_t)need * sizeof(float4)));
     cudaError_t e = cudaMalloc(&b, (size_t)(need / SB) * SBH * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&t, (size_t)need * sizeof(float2));
     if (e != cudaSuccess) {
         cudaFree(p);
+        if (b) cudaFree(b);
         return cuda_fail(c, e);
     }
     if (c->d_chg) cudaFree(c->d_chg);
     if (c->d_chg_blk) cudaFree(c->d_chg_blk);
+    if (c->d_trk) cudaFree(c->d_trk);
     c->d_chg = p;
     c->d_chg_blk = b;
+    c->d_trk = t;
     c->chg_cap = need;
     return OBEM_OK;
 }
@@ -878,7 +1024,7 @@ int grow_stage(obem_ctx* c, int i, size_t bytes)
 
 /* the evaluation proper: targets tgt[0..nt) -> out[0..nt) (declared in obem_internal.cuh) */
 int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
-                       float eps_nbody, cudaStream_t st)
+                       float eps_nbody, cudaStream_t st, float2* trk_out)
 {
     if (flags & ~(OBEM_NBODY | OBEM_PANELS)) return OBEM_EINVAL;
     if ((flags & OBEM_NBODY) && c->n_chg < 0) return OBEM_ESTATE;
@@ -928,6 +1074,8 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     P.bad_count = c->d_bad_count;
     P.bad_list = c->d_bad_list;
     P.accumulate = 0;
+    P.trk_out = trk_out;
+    P.trk_ws = c->d_trk_ws;
     OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
 
     /* one stream-K launch (+ fix-up) per section; the second adds to the first's result */
@@ -941,9 +1089,12 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
         Q.accumulate = (k > 0);
         if (Q.sec[0].kind == KIND_PANELS) {
             Q.self_first = -1;
-            obem_eval_kernel<KIND_PANELS><<<c->grid, THREADS, 0, st>>>(Q);
+            Q.trk_out = nullptr;
+            obem_eval_kernel<KIND_PANELS, false><<<c->grid, THREADS, 0, st>>>(Q);
+        } else if (Q.trk_out) {
+            obem_eval_kernel<KIND_POINTS, true><<<c->grid, THREADS, 0, st>>>(Q);
         } else {
-            obem_eval_kernel<KIND_POINTS><<<c->grid, THREADS, 0, st>>>(Q);
+            obem_eval_kernel<KIND_POINTS, false><<<c->grid, THREADS, 0, st>>>(Q);
         }
         OBEM_CUDA(c, cudaGetLastError());
         obem_fixup_kernel<<<(unsigned)Q.ntiles, THREADS, 0, st>>>(Q, c->grid);
@@ -981,7 +1132,7 @@ int obem_create(obem_ctx** out, int device)
     }
     c->sm_count = prop.multiProcessorCount;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<KIND_POINTS>, THREADS, 0);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<KIND_POINTS, true>, THREADS, 0);
     if (e != cudaSuccess || per_sm < 1) {
         /* no sm_100a code for this device, or the kernel cannot be resident */
         cudaGetLastError();
@@ -991,6 +1142,7 @@ int obem_create(obem_ctx** out, int device)
     if (per_sm > CTAS_PER_SM) per_sm = CTAS_PER_SM;
     c->grid = c->sm_count * per_sm;
     e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_trk_ws, (size_t)c->grid * 2 * TT * sizeof(float2));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_sink, 256);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_count, 256);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_list, (size_t)BAD_CAP * sizeof(long long));
@@ -1020,6 +1172,8 @@ int obem_destroy(obem_ctx* c)
     if (c->d_next_scratch) cudaFree(c->d_next_scratch);
     if (c->d_step_field) cudaFree(c->d_step_field);
     if (c->d_ws) cudaFree(c->d_ws);
+    if (c->d_trk_ws) cudaFree(c->d_trk_ws);
+    if (c->d_trk) cudaFree(c->d_trk);
     if (c->d_sink) cudaFree(c->d_sink);
     if (c->d_bad_count) cudaFree(c->d_bad_count);
     if (c->d_bad_list) cudaFree(c->d_bad_list);
@@ -1117,6 +1271,41 @@ int obem_eval_at_charges(obem_ctx* c, float* d_out, unsigned flags, void* cuda_s
     if (!c) return OBEM_EINVAL;
     if (c->n_chg < 0) return OBEM_ESTATE;
     return obem_eval_at_charges_range(c, 0, c->n_chg, d_out, flags, cuda_stream);
+}
+
+int obem_eval_at_charges_partners_range(obem_ctx* c, int64_t first, int64_t count, float* d_out, float* d_partner_d,
+                                        int32_t* d_partner_j, unsigned flags, void* cuda_stream)
+{
+    if (!c || first < 0 || count < 0) return OBEM_EINVAL;
+    if (c->n_chg < 0) return OBEM_ESTATE;
+    if (first + count > c->n_chg || !(flags & OBEM_NBODY)) return OBEM_EINVAL;
+    if (count > 0 && (!d_out || !d_partner_d || !d_partner_j || !aligned16(d_out) || !aligned4(d_partner_d) ||
+                      !aligned4(d_partner_j)))
+        return OBEM_EINVAL;
+    if (count == 0) return OBEM_OK;
+    DeviceGuard g(c->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int rc = obem_eval_internal(c, c->d_chg + first, count, (float4*)d_out, flags, first, c->eps_pp, st, c->d_trk);
+    if (rc != OBEM_OK) return rc;
+    partner_resolve_kernel<<<(unsigned)ceil_div(count, 8), 256, 0, st>>>(c->d_chg, c->d_chg_blk, c->d_trk, first, count,
+                                                                       c->n_chg, d_partner_d, d_partner_j);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return OBEM_OK;
+}
+
+int obem_eval_at_charges_partners(obem_ctx* c, float* d_out, float* d_partner_d, int32_t* d_partner_j, unsigned flags,
+                                  void* cuda_stream)
+{
+    if (!c) return OBEM_EINVAL;
+    if (c->n_chg < 0) return OBEM_ESTATE;
+    return obem_eval_at_charges_partners_range(c, 0, c->n_chg, d_out, d_partner_d, d_partner_j, flags, cuda_stream);
+}
+
+double obem_recombination_radius(double e_ioni_ev)
+{
+    /* Eq (3.12): d <= 1/(4 pi eps0) * e / (2 E_ioni); with E_ioni in eV the bound is k_e e / (2 E_ioni[V]) metres */
+    return (e_ioni_ev > 0.0) ? KE_D * 1.602176634e-19 / (2.0 * e_ioni_ev) : 0.0;
 }
 
 int obem_eval_at_points(obem_ctx* c, const float* d_pts, int64_t m, float* d_out, unsigned flags, void* cuda_stream)

@@ -132,6 +132,8 @@ struct obem_ctx {
     long long pan_cap = 0; /* capacity in panels */
     long long n_pan = -1;
     /* split-tile workspace [grid][2][TT] */
+    float2* d_trk = nullptr;     /* [chg_cap] (min softened r2 to an opposite charge, its source block) per charge */
+    float2* d_trk_ws = nullptr;  /* [grid][2][TT] the same for split tiles                                        */
     float4* d_ws = nullptr;
     float* d_sink = nullptr;
     unsigned* d_bad_count = nullptr;
@@ -186,8 +188,9 @@ bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
 
 /* The evaluation proper (obem.cu): targets tgt[0..nt) -> out[0..nt) on stream st.  self_first >= 0: target i IS
  * charge self_first + i and is excluded from its own N-body sum by index.  eps_nbody: softening of the N-body
- * section for this call (eval_at_*: eps_pp; influence on the cells: eps_panel). */
+ * section for this call (eval_at_*: eps_pp; influence on the cells: eps_panel).  trk_out != NULL (targets must be
+ * charges): also record, per target, the source block of its nearest opposite-sign charge (recombination). */
 int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
-                       float eps_nbody, cudaStream_t st);
+                       float eps_nbody, cudaStream_t st, float2* trk_out = nullptr);
 
 #endif /* OBEM_INTERNAL_CUH */

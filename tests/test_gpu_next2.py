@@ -172,3 +172,105 @@ def test_drift_kick_primitives_and_edge_cases(torch_cuda, api, ctx):
         ctx.step_euler(d_x, d_v, 1e-15, flags=api.PANELS)
     with pytest.raises(api.ObemError):
         ctx.step_pefrl(d_x, d_v, float("nan"), flags=api.NBODY)
+
+
+# --------------------------------------------------------------------------------------------------
+# recombination by-product of the N-body pass (Eq 3.12)
+# --------------------------------------------------------------------------------------------------
+def _check_partners(xyzq, eps, pd, pj, od, oj, idx=None, what=""):
+    """Distances must match the oracle up to the documented near-tie slack; the index must be the oracle's unless
+    another opposite charge sits within that slack (then it must be a valid opposite charge at the reported
+    distance)."""
+    pd = pd.astype(np.float64)
+    n = xyzq.shape[0]
+    idx = np.arange(n) if idx is None else idx
+    none = oj < 0
+    assert np.array_equal(pj[none], oj[none]) and np.all(np.isinf(pd[none])), what
+    has = ~none
+    d2_true = od[has] ** 2
+    slack = 4.0 * np.spacing((d2_true + eps * eps).astype(np.float32)).astype(np.float64)
+    assert np.all(pd[has] ** 2 <= d2_true * (1 + 3e-7) + slack), what
+    assert np.all(pd[has] >= od[has] * (1 - 1e-7)), what                   # never closer than the true nearest
+    # the reported index is a real opposite charge at the reported distance
+    tj = pj[has].astype(np.int64)
+    ti = idx[has]
+    assert np.all(tj >= 0) and np.all(tj < n) and np.all(tj != ti), what
+    assert np.all(xyzq[tj, 3] * xyzq[ti, 3] < 0), what
+    dd = np.linalg.norm(xyzq[tj, :3].astype(np.float64) - xyzq[ti, :3].astype(np.float64), axis=1)
+    assert np.allclose(dd, pd[has], rtol=2e-7, atol=0), what
+    same = tj == oj[has]
+    if same.size == 0:
+        return 1.0
+    assert same.mean() > 0.999, "%s: only %.4f of the partners are the oracle's" % (what, same.mean())
+    return float(same.mean())
+
+
+def test_partners_config1_and_field_unchanged(torch_cuda, api, ctx, ref):
+    from parity_metrics import assert_parity
+    torch = torch_cuda
+    wl = W.make_workload(1)
+    ctx.set_softening(wl.eps_pp, wl.eps_panel)
+    ctx.set_panels(dev(torch, wl.verts), dev(torch, wl.sigma))
+    ctx.set_charges(dev(torch, wl.xyzq))
+    out, pd, pj = ctx.eval_at_charges_partners(flags=api.NBODY | api.PANELS)
+    plain = ctx.eval_at_charges(flags=api.NBODY | api.PANELS)
+    torch.cuda.synchronize()
+    on, op = ref.eval_field(xyzq=wl.xyzq, verts=wl.verts, sigma=wl.sigma, eps_pp=wl.eps_pp, eps_panel=wl.eps_panel)
+    assert_parity(out.cpu().numpy(), on + op, "cfg1 field with partner tracking")
+    assert torch.equal(out, plain)                                       # the by-product does not change the field
+    od, oj = ref.nearest_opposite(wl.xyzq)
+    _check_partners(wl.xyzq, wl.eps_pp, pd.cpu().numpy(), pj.cpu().numpy(), od, oj, what="cfg1")
+
+
+@pytest.mark.parametrize("n,eps", [(3000, 0.1 * UM), (5000, 0.0), (1, 0.1 * UM), (300, 0.05 * UM)])
+def test_partners_mixed_signs(torch_cuda, api, ctx, ref, n, eps):
+    """Unsorted species, zero charges, doubly charged ions: every block is non-uniform (per-source sign test)."""
+    torch = torch_cuda
+    rng = np.random.default_rng([13, 7, n])
+    xyzq = np.zeros((n, 4), dtype=np.float32)
+    xyzq[:, :3] = rng.uniform(0, 50 * UM, (n, 3))
+    xyzq[:, 3] = rng.choice([-QE, QE, 2 * QE, 0.0], n, p=[0.45, 0.35, 0.1, 0.1])
+    ctx.set_softening(eps, 0.0)
+    ctx.set_charges(dev(torch, xyzq))
+    out, pd, pj = ctx.eval_at_charges_partners(flags=api.NBODY)
+    od, oj = ref.nearest_opposite(xyzq)
+    _check_partners(xyzq, eps, pd.cpu().numpy(), pj.cpu().numpy(), od, oj, what="mixed n=%d" % n)
+    # one species only: nobody has a partner
+    xyzq[:, 3] = -QE
+    ctx.set_charges(dev(torch, xyzq))
+    _, pd, pj = ctx.eval_at_charges_partners(flags=api.NBODY)
+    assert torch.all(pj == -1) and torch.all(torch.isinf(pd))
+
+
+def test_partners_config2_reduced_split_tiles_and_range(torch_cuda, api, ctx, ref):
+    torch = torch_cuda
+    wl = W.make_workload(2, charge_div=4, mesh_div=8)                    # 16384 charges: 8 tiles, split between CTAs
+    ctx.set_softening(wl.eps_pp, 0.0)
+    ctx.set_charges(dev(torch, wl.xyzq))
+    _, pd, pj = ctx.eval_at_charges_partners(flags=api.NBODY)
+    od, oj = ref.nearest_opposite(wl.xyzq)
+    _check_partners(wl.xyzq, wl.eps_pp, pd.cpu().numpy(), pj.cpu().numpy(), od, oj, what="cfg2/4")
+    first, count = 5000, 7001
+    _, pd2, pj2 = ctx.eval_at_charges_partners(flags=api.NBODY, first=first, count=count)
+    assert torch.equal(pj2, pj[first:first + count]) and torch.equal(pd2, pd[first:first + count])
+    with pytest.raises(api.ObemError):
+        ctx.eval_at_charges_partners(flags=api.PANELS)                   # the by-product needs the N-body pass
+
+
+def test_partners_config3_full_size_sampled(torch_cuda, api, ctx, ref):
+    torch = torch_cuda
+    wl = W.make_workload(3)
+    ctx.set_softening(wl.eps_pp, 0.0)
+    ctx.set_charges(dev(torch, wl.xyzq))
+    _, pd, pj = ctx.eval_at_charges_partners(flags=api.NBODY)
+    torch.cuda.synchronize()
+    pd, pj = pd.cpu().numpy(), pj.cpu().numpy()
+    rng = np.random.default_rng([13, 9])
+    idx = np.unique(np.concatenate([rng.choice(wl.n_charges, 2048, replace=False), np.argsort(pd)[:256],
+                                    np.argsort(pd)[-64:], [0, wl.n_charges - 1]]))
+    od, oj = ref.nearest_opposite(wl.xyzq, idx=idx)
+    _check_partners(wl.xyzq, wl.eps_pp, pd[idx], pj[idx], od, oj, idx=idx, what="cfg3 sampled")
+    # Eq (3.12): the mask a transport loop would apply
+    r = api.recombination_radius(15.76)
+    assert abs(r - ref.recombination_radius(15.76)) < 1e-24
+    assert np.array_equal(pd[idx] <= r, od <= r)

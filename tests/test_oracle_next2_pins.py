@@ -158,6 +158,9 @@ def test_r1_nearest_opposite_against_kdtree(ref):
         dd, jj = cKDTree(pos[other]).query(pos[mine], k=1)
         assert np.allclose(d[mine], dd, rtol=1e-13)
         assert np.array_equal(j[mine], other[jj])
+    sub = np.array([5, 17, 2999, 0, 1234])
+    ds, js = ref.nearest_opposite(xyzq, idx=sub)                          # subset form: same answers
+    assert np.array_equal(ds, d[sub]) and np.array_equal(js, j[sub])
     zero = np.where(q == 0)[0]
     assert np.all(j[zero] == -1) and np.all(np.isinf(d[zero]))
     assert not np.isin(j[j >= 0], zero).any()
