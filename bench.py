@@ -361,6 +361,7 @@ def run_ours(args):
     if world == 1 and not args.no_next:
         extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev)
         extras["next2"] = bench_next2(torch, api, ctx, wl, timed, dev, extras["nbody_only"]["s"])
+        extras["next4"] = bench_next4(torch, api, ctx, wl, timed, dev)
 
     # ---- roofline of the dominant kernel (obem_eval_kernel) -------------------------------------------
     sm_count = ctx.sm_count
@@ -480,6 +481,39 @@ def bench_next2(torch, api, ctx, wl, timed, dev, t_nbody):
     t_p = timed(lambda: ctx.step_pefrl(x, v, 25e-15), reps=1)
     res["step_pefrl"] = {"s": t_p, "field_evaluations": 4, "Ginteractions_per_s": 4 * per_eval / t_p / 1e9}
     ctx.set_charges(torch.from_numpy(wl.xyzq).to(dev))
+    return res
+
+
+def bench_next4(torch, api, ctx, wl, timed, dev):
+    """Static field option: trilinear interpolation in a 256^3 x float4 map (config 5's shape,
+    268 MB: larger than L2) at the bench workload's charges (clustered, as an avalanche is) and at as many
+    uniformly scattered positions (worst case for the gather).  HBM bound; algorithmic bytes = 16 B position in +
+    16 B result out per position + the map read once if every node is touched (scattered: min(map, 8 x 16 B x M))."""
+    n = wl.n_charges
+    shape = (256, 256, 256)
+    origin = (-210e-6, -210e-6, -150e-6)
+    spacing = (420e-6 / 255, 420e-6 / 255, 300e-6 / 255)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(4)
+    fmap = torch.empty(shape + (4,), dtype=torch.float32, device=dev)
+    fmap.normal_(0.0, 1.0, generator=gen)
+    pts_c = torch.from_numpy(wl.xyzq).to(dev)
+    pts_u = torch.rand((n, 4), dtype=torch.float32, device=dev, generator=gen)
+    pts_u = pts_u * torch.tensor([420e-6, 420e-6, 300e-6, 0.0], device=dev) + torch.tensor(
+        [origin[0], origin[1], origin[2], 0.0], device=dev)
+    out = torch.empty((n, 4), dtype=torch.float32, device=dev)
+    peak, src = hbm_peak_gbs()
+    res = {"map": "256x256x256 float4 (268 MB)", "positions": n, "bound": "hbm", "peak": peak, "unit": "GB/s",
+           "peak_source": src}
+    map_bytes = fmap.numel() * 4
+    for name, pts in (("at_charges", pts_c), ("scattered", pts_u)):
+        t = timed(lambda: ctx.interp_map(fmap, origin, spacing, pts, out=out), reps=5)
+        stream_b = 32 * n
+        touched = min(map_bytes, 8 * 16 * n)
+        res[name] = {"s": t, "Mpositions_per_s": n / t / 1e6, "streamed_GBps": stream_b / t / 1e9,
+                     "frac_streamed_only": stream_b / t / 1e9 / peak,
+                     "GBps_incl_map_upper_bound": (stream_b + touched) / t / 1e9}
+    del fmap
     return res
 
 

@@ -226,6 +226,29 @@ double obem_recombination_radius(double e_ioni_ev);
 /* Copy (n_x, n_y, n_z, A) of every panel to d_out [n_panels][4] fp32 -- inspection and tests. */
 int obem_get_panel_normals(obem_ctx* c, float* d_out, void* cuda_stream);
 
+/* ----------------------------------------------------------------------------------------------------------
+ * NEXT-4: the static field option, section 3.2.1: "the field components are computed only once at
+ * some predefined spatial coordinates located on a uniform 3D grid map ... During the transport, the field
+ * components at each particle location are then interpolated in this 3D map."
+ * Map: node (ix, iy, iz) at (o_x + ix d_x, o_y + iy d_y, o_z + iz d_z), 0 <= ix < nx ...; values
+ * d_map[((ix*ny + iy)*nz + iz)*4 + 0..3] = Ex, Ey, Ez [V/m], phi [V] (z fastest), caller-owned, 16-byte aligned.
+ * h_origin, h_spacing: HOST double[3] in metres; spacing > 0 along every axis with more than one node.
+ * ---------------------------------------------------------------------------------------------------------- */
+
+/* Fill the map: evaluate the sums `flags` selects (as obem_eval_at_points) at every node.  The node coordinate is
+ * the fp64 value o + i*d (one multiply, one add) rounded once to fp32.  The node list lives in a library-owned
+ * buffer that grows (cudaMalloc) on the first call of a given size. */
+int obem_field_map(obem_ctx* c, int nx, int ny, int nz, const double* h_origin, const double* h_spacing,
+                   float* d_map, unsigned flags, void* cuda_stream);
+
+/* Interpolate the map at d_pts [m][4] (4th lane ignored) into d_out [m][4]: trilinear in every component between
+ * the 8 surrounding nodes; positions outside the node lattice are clamped to its boundary (reading A18).  The cell
+ * index and fractions are taken in fp64, the 8-term weighted sum in fp32.  accumulate != 0: d_out += the
+ * interpolated value (static set-up field + N-body field), else d_out is overwritten. */
+int obem_interp_map(obem_ctx* c, const float* d_map, int nx, int ny, int nz, const double* h_origin,
+                    const double* h_spacing, const float* d_pts, int64_t m, float* d_out, int accumulate,
+                    void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

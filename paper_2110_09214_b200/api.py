@@ -16,6 +16,7 @@ PANELS = 2  # OBEM_PANELS -- Eq (2.13)/(2.14)
 
 _c_fp = ctypes.c_void_p  # device or host float* passed as an address
 _i64 = ctypes.c_int64
+_c_dp3 = ctypes.POINTER(ctypes.c_double)  # host double[3]
 
 # every symbol include/obem.h declares: name -> (restype, argtypes)
 SIGNATURES = {
@@ -65,6 +66,11 @@ SIGNATURES = {
                                        ctypes.c_void_p]),
     "obem_step_pefrl": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_uint,
                                        ctypes.c_void_p]),
+    # NEXT-4: static field option (map + trilinear interpolation)
+    "obem_field_map": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_dp3, _c_dp3,
+                                      _c_fp, ctypes.c_uint, ctypes.c_void_p]),
+    "obem_interp_map": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_dp3,
+                                       _c_dp3, _c_fp, _i64, _c_fp, ctypes.c_int, ctypes.c_void_p]),
 }
 
 LIB_PATH = _build.LIB
@@ -436,6 +442,44 @@ class Context:
             self._h, int(first), int(count), out.data_ptr() if ok else None, pd.data_ptr() if ok else None,
             pj.data_ptr() if ok else None, int(flags), _stream_ptr(stream)), "obem_eval_at_charges_partners_range")
         return out, pd, pj
+
+    # -- NEXT-4: static field option ------------------------------------------------------
+    def field_map(self, shape, origin, spacing, flags: int = PANELS, out=None, stream=None):
+        """Fill a [nx, ny, nz, 4] map (Ex, Ey, Ez, phi at the nodes origin + i*spacing)."""
+        nx, ny, nz = (int(v) for v in shape)
+        if out is None:
+            out = self._new((nx, ny, nz, 4))
+        else:
+            _dev_f32(out, "out", (nx, ny, nz, 4))
+        o = (ctypes.c_double * 3)(*[float(v) for v in origin])
+        d = (ctypes.c_double * 3)(*[float(v) for v in spacing])
+        self._check(_lib.obem_field_map(self._h, nx, ny, nz, o, d, out.data_ptr(), int(flags), _stream_ptr(stream)),
+                    "obem_field_map")
+        return out
+
+    def interp_map(self, fmap, origin, spacing, pts, out=None, accumulate: bool = False, stream=None):
+        """Trilinear interpolation of fmap [nx, ny, nz, 4] at pts [M, 4] -> [M, 4] (added to `out` if accumulate)."""
+        _dev_f32(fmap, "fmap", (4,))
+        if fmap.dim() != 4:
+            raise ValueError("fmap must be [nx, ny, nz, 4]")
+        nx, ny, nz = (int(v) for v in fmap.shape[:3])
+        m = int(pts.shape[0])
+        if m:
+            _dev_f32(pts, "pts", (4,))
+        if out is None:
+            if accumulate:
+                raise ValueError("accumulate needs an `out` to add to")
+            out = self._new((m, 4))
+        elif m:
+            _dev_f32(out, "out", (4,))
+            if out.shape[0] != m:
+                raise ValueError("out and pts disagree on the number of positions")
+        o = (ctypes.c_double * 3)(*[float(v) for v in origin])
+        d = (ctypes.c_double * 3)(*[float(v) for v in spacing])
+        self._check(_lib.obem_interp_map(self._h, fmap.data_ptr(), nx, ny, nz, o, d, pts.data_ptr() if m else None,
+                                         m, out.data_ptr() if m else None, 1 if accumulate else 0,
+                                         _stream_ptr(stream)), "obem_interp_map")
+        return out
 
 
 def recombination_radius(e_ioni_ev: float) -> float:

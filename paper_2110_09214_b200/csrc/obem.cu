@@ -1171,6 +1171,7 @@ int obem_destroy(obem_ctx* c)
     if (c->d_qrel) cudaFree(c->d_qrel);
     if (c->d_next_scratch) cudaFree(c->d_next_scratch);
     if (c->d_step_field) cudaFree(c->d_step_field);
+    if (c->d_map_pts) cudaFree(c->d_map_pts);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_trk_ws) cudaFree(c->d_trk_ws);
     if (c->d_trk) cudaFree(c->d_trk);

@@ -150,6 +150,9 @@ struct obem_ctx {
     int gemv_attr_set = 0;
     float4* d_step_field = nullptr; /* [n] E, phi at the charges: scratch of the steppers */
     long long step_field_cap = 0;
+    /* obem_map.cu */
+    float4* d_map_pts = nullptr; /* node coordinates of the last obem_field_map */
+    size_t map_pts_cap = 0;      /* bytes */
 };
 
 namespace {
