@@ -145,10 +145,13 @@ def oracle_sample_rate(wl, seconds: float, seed: int = 123):
     probe = np.sort(rng.choice(nt, min(nt, 4 * cores), replace=False))
     tp = max(run(probe), 1e-6)
     rate = len(probe) * per_target / tp
-    n_s = int(min(nt, max(len(probe), seconds * rate / per_target)))
-    idx = np.sort(rng.choice(nt, n_s, replace=False))
-    ts = run(idx)
-    rate = n_s * per_target / ts
+    for _ in range(2):  # the small probe underestimates the rate (thread start-up): re-size once from a real run
+        n_s = int(min(nt, max(len(probe), seconds * rate / per_target)))
+        idx = np.sort(rng.choice(nt, n_s, replace=False))
+        ts = run(idx)
+        rate = n_s * per_target / ts
+        if ts >= 0.6 * seconds or n_s == nt:
+            break
     desc = "%d seeded targets of %d against all %d charges + %d panels (%.3g interactions, %.1f s)" % (
         n_s, nt, wl.n_charges, wl.n_panels, n_s * per_target, ts)
     return rate, cores, desc, ts

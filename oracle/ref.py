@@ -17,7 +17,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "obem_ref.c")
-_SRCS = [_SRC, os.path.join(_HERE, "obem_ref_next.c")]   # hot path; adjacent steps
+_SRCS = [_SRC, os.path.join(_HERE, "obem_ref_next.c"),   # hot path; adjacent steps
+         os.path.join(_HERE, "obem_ref_analytic.c")]       # NEXT-3: exact cell integrals
 _LIB = os.path.join(_HERE, "libobem_ref.so")
 
 NBODY = 1
@@ -69,6 +70,11 @@ def _load():
         lib.obem_ref_recombination_radius.argtypes = [ctypes.c_double]
         lib.obem_ref_matvec.restype = ctypes.c_int
         lib.obem_ref_matvec.argtypes = [c_fp, ctypes.c_int64, ctypes.c_int64, c_fp, c_dp, ctypes.c_int]
+        lib.obem_ref_tri_integrals.restype = None
+        lib.obem_ref_tri_integrals.argtypes = [c_dp, c_dp, c_dp, c_dp, c_dp, c_dp]
+        lib.obem_ref_eval_panels_analytic.restype = ctypes.c_int
+        lib.obem_ref_eval_panels_analytic.argtypes = [c_fp, c_fp, ctypes.c_int64, c_fp, ctypes.c_int64, c_dp,
+                                                      ctypes.c_int]
         _lib = lib
     return _lib
 
@@ -222,3 +228,32 @@ def nearest_opposite(xyzq, idx=None, n_threads: int = 0):
 def recombination_radius(e_ioni_ev: float) -> float:
     """Eq (3.12): k_e e / (2 E_ioni) in metres, E_ioni in eV."""
     return float(_load().obem_ref_recombination_radius(float(e_ioni_ev)))
+
+
+# --------------------------------------------------------------------------------------------------
+# NEXT-3 (SURVEY.md 8f): exact cell integrals of Eq (2.13)/(2.14) over flat triangles (obem_ref_analytic.c)
+# --------------------------------------------------------------------------------------------------
+def tri_integrals(v0, v1, v2, r):
+    """(I_phi, I_E[3]) = (Int dS/R, Int (r - r')/R^3 dS) over the flat triangle (v0, v1, v2) at r; float64."""
+    a = [np.ascontiguousarray(x, dtype=np.float64).reshape(3) for x in (v0, v1, v2, r)]
+    iphi = np.zeros(1, dtype=np.float64)
+    ie = np.zeros(3, dtype=np.float64)
+    _load().obem_ref_tri_integrals(*[_ptr(x, ctypes.c_double) for x in a], _ptr(iphi, ctypes.c_double),
+                                   _ptr(ie, ctypes.c_double))
+    return float(iphi[0]), ie
+
+
+def eval_panels_analytic(verts, sigma, targets, n_threads: int = 0):
+    """k_e sum_p sigma_p (I_E, I_phi) at every target: [T, 4] float64 = Ex, Ey, Ez, phi."""
+    verts = _f32(verts, (3, 3))
+    sigma = _f32(sigma, ())
+    targets = _f32(targets, (4,))
+    npan, nt = verts.shape[0], targets.shape[0]
+    assert sigma.shape[0] == npan
+    out = np.zeros((nt, 4), dtype=np.float64)
+    rc = _load().obem_ref_eval_panels_analytic(_ptr(verts, ctypes.c_float), _ptr(sigma, ctypes.c_float), npan,
+                                               _ptr(targets, ctypes.c_float), nt, _ptr(out, ctypes.c_double),
+                                               int(n_threads))
+    if rc != 0:
+        raise ValueError("obem_ref_eval_panels_analytic: bad argument")
+    return out
