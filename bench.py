@@ -364,6 +364,7 @@ def run_ours(args):
     if world == 1 and not args.no_next:
         extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev)
         extras["next2"] = bench_next2(torch, api, ctx, wl, timed, dev, extras["nbody_only"]["s"])
+        extras["next3"] = bench_next3(torch, api, ctx, wl, timed, out, extras["panels_only"]["s"])
         extras["next4"] = bench_next4(torch, api, ctx, wl, timed, dev)
 
     # ---- roofline of the dominant kernel (obem_eval_kernel) -------------------------------------------
@@ -485,6 +486,22 @@ def bench_next2(torch, api, ctx, wl, timed, dev, t_nbody):
     res["step_pefrl"] = {"s": t_p, "field_evaluations": 4, "Ginteractions_per_s": 4 * per_eval / t_p / 1e9}
     ctx.set_charges(torch.from_numpy(wl.xyzq).to(dev))
     return res
+
+
+def bench_next3(torch, api, ctx, wl, timed, out, t_panels):
+    """Near-field-accurate panels: the panel sum with the closed-form integrals for the panels
+    within 3 longest-edges of each charge, against the 7-point sum alone.  The first call builds the cell lists
+    (once per geometry) and is timed separately."""
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    ctx.eval_at_charges(out=out, flags=api.PANELS | api.PANELS_EXACT)
+    ev1.record()
+    torch.cuda.synchronize()
+    t_first = ev0.elapsed_time(ev1) * 1e-3
+    t_ex = timed(lambda: ctx.eval_at_charges(out=out, flags=api.PANELS | api.PANELS_EXACT))
+    return {"panels_exact": {"s": t_ex, "overhead_vs_7_point_only": t_ex / t_panels - 1.0,
+                             "first_call_with_list_build_s": t_first, "near_factor": 3.0,
+                             "cell_list_entries": ctx.near_list_size, "cells": ctx.near_cells}}
 
 
 def bench_next4(torch, api, ctx, wl, timed, dev):

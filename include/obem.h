@@ -58,6 +58,7 @@ typedef enum obem_status {
 /* flags of the evaluate calls: which of the two sums to include */
 #define OBEM_NBODY 1u  /* Eq (3.8), sources = the charges of obem_set_charges              */
 #define OBEM_PANELS 2u /* Eq (2.13)/(2.14), sources = the panels of obem_set_panels         */
+#define OBEM_PANELS_EXACT 4u /* with OBEM_PANELS: exact cell integrals near the target, see obem_set_near_field */
 
 /* Create a context on CUDA device `device`.  Queries the SM count and sizes the persistent grid.
  * *out is NULL on failure. */
@@ -225,6 +226,28 @@ double obem_recombination_radius(double e_ioni_ev);
 
 /* Copy (n_x, n_y, n_z, A) of every panel to d_out [n_panels][4] fp32 -- inspection and tests. */
 int obem_get_panel_normals(obem_ctx* c, float* d_out, void* cuda_stream);
+
+/* ----------------------------------------------------------------------------------------------------------
+ * NEXT-3: near-field-accurate panels.  PAPER.md:131-133, :147: "the corresponding integrals are calculated
+ * analytically".  The 7-point rule of the hot path differs from the exact integral of Eq (2.13)/(2.14) by
+ * ~(h/r)^6 (2.7e-3 of the panel's own field at r = h, 2.5e-5 at 2h, 2.1e-6 at 3h, 3.8e-7 at 4h; h = longest
+ * edge, r = distance to the centroid).  With OBEM_PANELS | OBEM_PANELS_EXACT every evaluate call (and every
+ * stepper) replaces, for each target, the 7-point value of each panel whose centroid is closer than
+ * near_factor * h_p by the closed-form integral over the flat triangle (fp64, edge-wise log / atan terms), so the
+ * result is Eq (2.13)/(2.14) itself to the tolerance of the path.  On a panel (d = 0) the normal component is the
+ * principal value 0 (reading A8); exactly on an edge the singular edge term is dropped (like reading A4).
+ * How: a uniform cell grid over the panels' near spheres (built on the first such call after obem_set_panels:
+ * allocates and synchronises once per geometry; obem_set_sigma keeps it), one warp per target scanning its cell's
+ * candidate list, near pairs compacted across the warp; the correction (exact - 7-point) is summed in fp64 in a
+ * fixed order and added to d_out.
+ * ---------------------------------------------------------------------------------------------------------- */
+
+/* near_factor > 0 and finite (default 3).  Takes effect at the next evaluate call (the cell lists are rebuilt). */
+int obem_set_near_field(obem_ctx* c, float near_factor);
+
+/* Number of (cell, panel) entries of the current cell lists and number of cells; -1 before the first build. */
+int64_t obem_near_list_size(const obem_ctx* c);
+int64_t obem_near_cells(const obem_ctx* c);
 
 /* ----------------------------------------------------------------------------------------------------------
  * NEXT-4: the static field option, section 3.2.1: "the field components are computed only once at

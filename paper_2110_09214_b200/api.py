@@ -13,6 +13,7 @@ from . import build as _build
 
 NBODY = 1   # OBEM_NBODY  -- Eq (3.8)
 PANELS = 2  # OBEM_PANELS -- Eq (2.13)/(2.14)
+PANELS_EXACT = 4  # OBEM_PANELS_EXACT -- with PANELS: closed-form cell integrals near the target (NEXT-3)
 
 _c_fp = ctypes.c_void_p  # device or host float* passed as an address
 _i64 = ctypes.c_int64
@@ -66,6 +67,10 @@ SIGNATURES = {
                                        ctypes.c_void_p]),
     "obem_step_pefrl": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _i64, ctypes.c_float, ctypes.c_uint,
                                        ctypes.c_void_p]),
+    # NEXT-3: near-field-accurate panels
+    "obem_set_near_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
+    "obem_near_list_size": (_i64, [ctypes.c_void_p]),
+    "obem_near_cells": (_i64, [ctypes.c_void_p]),
     # NEXT-4: static field option (map + trilinear interpolation)
     "obem_field_map": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_dp3, _c_dp3,
                                       _c_fp, ctypes.c_uint, ctypes.c_void_p]),
@@ -442,6 +447,18 @@ class Context:
             self._h, int(first), int(count), out.data_ptr() if ok else None, pd.data_ptr() if ok else None,
             pj.data_ptr() if ok else None, int(flags), _stream_ptr(stream)), "obem_eval_at_charges_partners_range")
         return out, pd, pj
+
+    # -- NEXT-3: near-field-accurate panels -------------------------------------------
+    def set_near_field(self, near_factor: float = 3.0):
+        self._check(_lib.obem_set_near_field(self._h, float(near_factor)), "obem_set_near_field")
+
+    @property
+    def near_list_size(self) -> int:
+        return int(_lib.obem_near_list_size(self._h))
+
+    @property
+    def near_cells(self) -> int:
+        return int(_lib.obem_near_cells(self._h))
 
     # -- NEXT-4: static field option ------------------------------------------------------
     def field_map(self, shape, origin, spacing, flags: int = PANELS, out=None, stream=None):

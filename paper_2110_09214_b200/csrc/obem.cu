@@ -1026,10 +1026,15 @@ int grow_stage(obem_ctx* c, int i, size_t bytes)
 int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                        float eps_nbody, cudaStream_t st, float2* trk_out)
 {
-    if (flags & ~(OBEM_NBODY | OBEM_PANELS)) return OBEM_EINVAL;
+    if (flags & ~(OBEM_NBODY | OBEM_PANELS | OBEM_PANELS_EXACT)) return OBEM_EINVAL;
+    if ((flags & OBEM_PANELS_EXACT) && !(flags & OBEM_PANELS)) return OBEM_EINVAL;
     if ((flags & OBEM_NBODY) && c->n_chg < 0) return OBEM_ESTATE;
     if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
     if (nt == 0) return OBEM_OK;
+    /* NEXT-3: exact integrals for the panels near each target (obem_near.cu) */
+    if ((flags & OBEM_PANELS_EXACT) && c->n_pan > 0)
+        return obem_eval_exact(c, tgt, nt, out, flags & ~OBEM_PANELS_EXACT, self_first, eps_nbody, st, trk_out);
+    flags &= ~OBEM_PANELS_EXACT;
 
     EvalParams P;
     int ns = 0;
@@ -1107,6 +1112,21 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     return OBEM_OK;
 }
 
+__global__ void panel_origins_kernel(const float4* __restrict__ src, float4* __restrict__ out, long long np)
+{
+    const long long p = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < np) out[p] = src[panel_entry(p)];
+}
+
+int obem_panel_origins(obem_ctx* c, float4* out, cudaStream_t st)
+{
+    if (c->n_pan <= 0) return OBEM_OK;
+    panel_origins_kernel<<<(unsigned)ceil_div(c->n_pan, 256), 256, 0, st>>>(c->d_psrc, out, c->n_pan);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    return OBEM_OK;
+}
+
 extern "C" {
 
 int obem_create(obem_ctx** out, int device)
@@ -1172,6 +1192,7 @@ int obem_destroy(obem_ctx* c)
     if (c->d_next_scratch) cudaFree(c->d_next_scratch);
     if (c->d_step_field) cudaFree(c->d_step_field);
     if (c->d_map_pts) cudaFree(c->d_map_pts);
+    obem_near_free(c);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_trk_ws) cudaFree(c->d_trk_ws);
     if (c->d_trk) cudaFree(c->d_trk);
@@ -1220,7 +1241,7 @@ int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int
         c->launches += 1;
     }
     c->n_pan = n_panels;
-    return OBEM_OK;
+    return obem_near_store_panels(c, d_verts, d_sigma, n_panels, st);
 }
 
 int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cuda_stream)
@@ -1235,7 +1256,7 @@ int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cu
         d_sigma, c->d_area, c->d_qrel, c->d_psrc, n_panels);
     OBEM_CUDA(c, cudaGetLastError());
     c->launches += 1;
-    return OBEM_OK;
+    return obem_near_store_sigma(c, d_sigma, n_panels, (cudaStream_t)cuda_stream);
 }
 
 int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_stream)

@@ -150,6 +150,29 @@ struct obem_ctx {
     int gemv_attr_set = 0;
     float4* d_step_field = nullptr; /* [n] E, phi at the charges: scratch of the steppers */
     long long step_field_cap = 0;
+    /* obem_near.cu: exact near-field panel integrals (NEXT-3) */
+    float* d_pverts = nullptr;   /* [np][3][3] copy of the vertices given to obem_set_panels            */
+    float* d_psigma = nullptr;   /* [np] copy of the current sigma                                       */
+    float4* d_porg = nullptr;    /* [np] frame origin of every panel (what the evaluation kernel shifts by) */
+    float4* d_pcr = nullptr;     /* [np] centroid and near radius R_p = near_factor * longest edge        */
+    long long near_cap = 0;      /* capacity of the four arrays above, in panels                         */
+    int* d_cell_start = nullptr; /* [ncells + 1] CSR offsets of the per-cell candidate lists             */
+    int* d_cell_fill = nullptr;  /* [ncells] fill cursors (build only)                                   */
+    int* d_cell_list = nullptr;  /* panels whose near sphere overlaps the cell, ascending                */
+    long long cell_cap = 0, list_cap = 0;
+    double* d_near_red = nullptr; /* [8] bounding box of the near spheres, sum and count of R (build only) */
+    void* d_scan_tmp = nullptr;
+    size_t scan_tmp_cap = 0;
+    double near_lo[3] = {0, 0, 0}, near_s = 0; /* grid origin and cell edge [m]                          */
+    int near_n[3] = {0, 0, 0};                 /* cells per axis; 0 = no cell (no panel has R > 0)       */
+    float near_factor = 3.0f;
+    int near_valid = 0; /* the grid matches the current panels and near_factor */
+    int* d_redo_list = nullptr;       /* targets too close to a quadrature source: recomputed in fp64 */
+    unsigned* d_redo_count = nullptr;
+    long long redo_cap = 0;
+    float4* d_exact_tmp = nullptr;    /* [nt] panel part of an N-body + exact-panels evaluation */
+    long long exact_tmp_cap = 0;
+    long long near_entries = -1; /* (cell, panel) entries of the current lists; -1 before the first build */
     /* obem_map.cu */
     float4* d_map_pts = nullptr; /* node coordinates of the last obem_field_map */
     size_t map_pts_cap = 0;      /* bytes */
@@ -195,5 +218,20 @@ bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
  * charges): also record, per target, the source block of its nearest opposite-sign charge (recombination). */
 int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                        float eps_nbody, cudaStream_t st, float2* trk_out = nullptr);
+
+/* obem.cu: copy the frame origin of every panel (what panel_loop shifts the targets by) to out[0..n_pan). */
+int obem_panel_origins(obem_ctx* c, float4* out, cudaStream_t st);
+
+/* obem_near.cu.  Called by obem_set_panels / obem_set_sigma: keep a copy of the geometry and of sigma for the exact
+ * near-field integrals.  obem_near_correct: out[t] += k_e sum over panels p near target t of sigma_p (exact cell
+ * integral - the 7-point value the evaluation kernel already added); builds the cell lists first if they are stale
+ * (allocates and synchronises: once per geometry).  obem_near_free: release everything (obem_destroy). */
+int obem_near_store_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, long long np, cudaStream_t st);
+int obem_near_store_sigma(obem_ctx* c, const float* d_sigma, long long np, cudaStream_t st);
+int obem_near_correct(obem_ctx* c, const float4* tgt, long long nt, float4* out, cudaStream_t st);
+/* the evaluation with OBEM_PANELS_EXACT: N-body part (if asked) into out, panel part + correction into scratch, sum */
+int obem_eval_exact(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
+                    float eps_nbody, cudaStream_t st, float2* trk_out);
+void obem_near_free(obem_ctx* c);
 
 #endif /* OBEM_INTERNAL_CUH */
