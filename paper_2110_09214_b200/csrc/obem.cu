@@ -55,6 +55,7 @@ constexpr int UNR = OBEM_UNR;         /* sources per unrolled inner-loop trip   
 constexpr int DEPTH = OBEM_DEPTH;     /* software-pipeline distance (work items) between the rsqrt
                                          of an item and its use                                     */
 static_assert(TPT % 2 == 0 && SB % UNR == 0, "bad tuning knobs");
+static_assert(SB == OBEM_SB && SB + 1 == OBEM_SBH && TT == OBEM_TT, "obem_internal.cuh states the block layout for obem_nn.cu");
 
 /* k_e = 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m (CODATA 2018), reading A7 */
 constexpr double KE_D = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12);
@@ -101,6 +102,14 @@ struct EvalParams {
     float2* trk_out;      /* TRACK: [nt] (min softened r2 over opposite-sign sources, its block index as int bits) */
     float2* trk_ws;       /* TRACK: [grid][2][TT] the same for split tiles                                  */
     int accumulate;       /* 1: add to what out already holds (the second section's launch)              */
+    /* LIST mode (the NN approximation, obem_nn.cu): the units of tile t are list[tile_ptr[t] .. tile_ptr[t+1]),
+     * each the index of a KIND_POINTS block in `pool` (stride SBH); U = tile_ptr[ntiles].  Blocks below
+     * list_self_blocks are blocks of the (sorted) charges themselves: block b holds sources [b SB, (b+1) SB). */
+    const long long* tile_ptr;
+    const int* list;
+    const float4* pool;
+    long long list_self_blocks;
+    const long long* U_dev; /* LIST: the unit count lives on the device (no host round trip when the lists are built) */
     unsigned* bad_count;  /* number of targets whose result came out non-finite (see obem_repair_kernel) */
     long long* bad_list;  /* their indices, at most BAD_CAP                                               */
 };
@@ -385,9 +394,22 @@ __device__ __forceinline__ unsigned unit_bytes(const EvalParams& P, long long bl
 /* One launch per source section: KIND selects the loops compiled in (P.sec[0] is the section; P.sec[1] is empty).
  * Two instantiations instead of one kernel with both loop families: each hot loop gets its own register
  * allocation (a combined kernel cost the uniform N-body loop 8 extra MOVs per trip, -4 %). */
-template <int KIND, bool TRACK>
+/* tile whose unit range [tile_ptr[t], tile_ptr[t+1]) contains u (LIST mode; empty tiles are skipped) */
+__device__ __forceinline__ long long list_tile_of(const long long* __restrict__ tile_ptr, long long ntiles, long long u)
+{
+    long long lo = 0, hi = ntiles - 1;
+    while (lo < hi) {
+        const long long mid = (lo + hi + 1) >> 1;
+        if (tile_ptr[mid] <= u) lo = mid;
+        else hi = mid - 1;
+    }
+    return lo;
+}
+
+template <int KIND, bool TRACK, bool LIST = false>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
 {
+    static_assert(!LIST || (KIND == KIND_POINTS && !TRACK), "LIST mode: point sources, no partner tracking");
     __shared__ __align__(128) float4 ring[STAGES][KIND == KIND_PANELS ? SBH_P : SBH + 3]; /* stage stride % 64 B == 0 */
     __shared__ __align__(8) u64 full[STAGES];
     /* TRACK: running (min r2, block) per target slot, updated once per block */
@@ -396,7 +418,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
 
     const int tid = threadIdx.x;
     const long long G = gridDim.x, c = blockIdx.x;
-    const long long u0 = unit_begin(c, P.U, G), u1 = unit_begin(c + 1, P.U, G);
+    const long long Utot = LIST ? *P.U_dev : P.U;
+    const long long u0 = unit_begin(c, Utot, G), u1 = unit_begin(c + 1, Utot, G);
     if (u0 >= u1) return;
 
     if (tid == 0) {
@@ -406,11 +429,16 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
     __syncthreads();
 
     /* producer state (thread 0): next unit to load and its source block */
-    long long pu = u0, pblk = u0 % P.nblk;
+    long long pu = u0, pblk = LIST ? 0 : u0 % P.nblk;
     if (tid == 0) {
         for (int s = 0; s < STAGES - 1 && pu < u1; ++s) {
-            mbar_expect_tx(&full[s], unit_bytes(P, pblk));
-            tma_load_1d(&ring[s][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[s]);
+            if (LIST) {
+                mbar_expect_tx(&full[s], (unsigned)(SBH * sizeof(float4)));
+                tma_load_1d(&ring[s][0], P.pool + (long long)P.list[pu] * SBH, (unsigned)(SBH * sizeof(float4)), &full[s]);
+            } else {
+                mbar_expect_tx(&full[s], unit_bytes(P, pblk));
+                tma_load_1d(&ring[s][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[s]);
+            }
             ++pu;
             if (++pblk == P.nblk) pblk = 0;
         }
@@ -420,10 +448,16 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
 
     long long u = u0;
     unsigned it = 0; /* units consumed so far by this CTA: stage = it % STAGES, parity = (it / STAGES) & 1 */
+    long long ltile = LIST ? list_tile_of(P.tile_ptr, P.ntiles, u0) : 0;
     while (u < u1) {
-        const long long tile = u / P.nblk;
-        const long long b0 = u - tile * P.nblk;
-        const long long nrun = min(P.nblk - b0, u1 - u);
+        if (LIST) {
+            while (P.tile_ptr[ltile + 1] <= u) ++ltile; /* next non-empty tile */
+        }
+        const long long tile = LIST ? ltile : u / P.nblk;
+        const long long tile_u0 = LIST ? P.tile_ptr[tile] : tile * P.nblk;
+        const long long tile_u1 = LIST ? P.tile_ptr[tile + 1] : tile_u0 + P.nblk;
+        const long long b0 = u - tile_u0;
+        const long long nrun = min(tile_u1 - u, u1 - u);
         const long long tbase = tile * (long long)TT + tid;
 
         u64 X[NPAIR], Y[NPAIR], Z[NPAIR];
@@ -458,13 +492,21 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
         /* source-index range of this tile's own targets inside sec[0] (evaluation at the charges) */
         const long long self_lo = (P.self_first >= 0) ? P.self_first + tile * (long long)TT : -1;
 
+        int next_blk = LIST ? __ldg(P.list + u) : 0;
         for (long long r = 0; r < nrun; ++r, ++it) {
-            const long long blk = b0 + r;
+            const long long blk = LIST ? (long long)next_blk : b0 + r;
+            if (LIST && r + 1 < nrun) next_blk = __ldg(P.list + u + r + 1); /* one block ahead: off the critical path */
             __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
             if (tid == 0 && pu < u1) {
                 const int ps = (it + STAGES - 1) % STAGES;
-                mbar_expect_tx(&full[ps], unit_bytes(P, pblk));
-                tma_load_1d(&ring[ps][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[ps]);
+                if (LIST) {
+                    mbar_expect_tx(&full[ps], (unsigned)(SBH * sizeof(float4)));
+                    tma_load_1d(&ring[ps][0], P.pool + (long long)P.list[pu] * SBH, (unsigned)(SBH * sizeof(float4)),
+                                &full[ps]);
+                } else {
+                    mbar_expect_tx(&full[ps], unit_bytes(P, pblk));
+                    tma_load_1d(&ring[ps][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[ps]);
+                }
                 ++pu;
                 if (++pblk == P.nblk) pblk = 0;
             }
@@ -487,7 +529,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
 #pragma unroll
                     for (int k = 0; k < TPT; ++k) bm[k] = __int_as_float(0x7f800000);
                 }
-                const bool diag = self_lo >= 0 && blk * SB < self_lo + TT && (blk + 1) * SB > self_lo;
+                const bool diag = self_lo >= 0 && (!LIST || blk < P.list_self_blocks) && blk * SB < self_lo + TT &&
+                                  (blk + 1) * SB > self_lo;
                 if (diag || (TRACK && !(blkw == blkw))) {
                     self_block_loop<TRACK>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP,
                                            diag ? self_lo + tid - blk * SB : -(1LL << 40), THREADS, bm, negmask, posmask);
@@ -517,7 +560,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             }
         }
 
-        const bool whole = (b0 == 0 && nrun == P.nblk);
+        const bool whole = (b0 == 0 && u + nrun == tile_u1);
         float4* wsl = P.ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT + tid;
 #pragma unroll
         for (int p = 0; p < NPAIR; ++p) {
@@ -603,10 +646,20 @@ __device__ __forceinline__ long long cta_of(long long u, long long U, long long 
 __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P, const int G)
 {
     const long long tile = blockIdx.x;
-    const long long uA = tile * P.nblk, uB = uA + P.nblk - 1;
-    const long long cA = cta_of(uA, P.U, G), cB = cta_of(uB, P.U, G);
-    if (cA == cB) return; /* one CTA had the whole tile and wrote it directly */
+    const bool LIST = P.list != nullptr;
+    const long long Utot = LIST ? *P.U_dev : P.U;
+    const long long uA = LIST ? P.tile_ptr[tile] : tile * P.nblk;
+    const long long uB = (LIST ? P.tile_ptr[tile + 1] : uA + P.nblk) - 1;
     const int tid = threadIdx.x;
+    if (uB < uA) { /* LIST: a tile with no unit at all */
+        for (int k = 0; k < TPT; ++k) {
+            const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
+            if (i < P.nt && !P.accumulate) P.out[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        return;
+    }
+    const long long cA = cta_of(uA, Utot, G), cB = cta_of(uB, Utot, G);
+    if (cA == cB) return; /* one CTA had the whole tile and wrote it directly */
     for (int k = 0; k < TPT; ++k) {
         const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
         if (i >= P.nt) continue;
@@ -614,9 +667,9 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
         float tm = __int_as_float(0x7f800000);
         int tb = -1;
         for (long long c = cA; c <= cB; ++c) {
-            const long long c0 = unit_begin(c, P.U, G), c1 = unit_begin(c + 1, P.U, G);
+            const long long c0 = unit_begin(c, Utot, G), c1 = unit_begin(c + 1, Utot, G);
             if (c0 >= c1) continue;
-            const int slot = (c0 / P.nblk == tile) ? 0 : 1;
+            const int slot = (c0 >= uA && c0 <= uB) ? 0 : 1; /* the CTA's range STARTS inside this tile */
             if (P.trk_out) { /* CTAs in ascending block order: strict < keeps the lowest block on ties */
                 const float2 t = P.trk_ws[((size_t)c * 2 + slot) * TT + (size_t)k * THREADS + tid];
                 if (t.x < tm) {
@@ -712,7 +765,24 @@ __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P
         for (int sct = 0; sct < 2; ++sct) {
             const Section& S = P.sec[sct];
             const double e2 = (double)S.eps2;
-            if (S.kind == KIND_POINTS) {
+            if (P.list != nullptr) {
+                if (sct != 0) continue;
+                /* LIST mode: the sources of target i are the blocks of its tile's list */
+                const long long tl = i / TT, self = P.self_first >= 0 ? P.self_first + i : -1;
+                for (long long j = P.tile_ptr[tl] * SB + tid; j < P.tile_ptr[tl + 1] * SB; j += THREADS) {
+                    const long long blk = P.list[j / SB];
+                    const float4 q = P.pool[blk * SBH + 1 + (j % SB)];
+                    if ((blk < P.list_self_blocks && blk * SB + (j % SB) == self) || q.w == 0.0f) continue;
+                    const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
+                    const double r2 = dx * dx + dy * dy + dz * dz + e2;
+                    if (!(r2 > 0.0)) continue;
+                    const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
+                    ph += w;
+                    ex += s3 * dx;
+                    ey += s3 * dy;
+                    ez += s3 * dz;
+                }
+            } else if (S.kind == KIND_POINTS) {
                 const long long self = (sct == 0 && P.self_first >= 0) ? P.self_first + i : -1;
                 for (long long j = tid; j < S.nblk * SB; j += THREADS) {
                     const float4 q = S.src[(j / SB) * SBH + 1 + (j % SB)];
@@ -1046,6 +1116,11 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     P.sec[0].npan = P.sec[1].npan = 0;
     P.sec[0].stride = P.sec[1].stride = SBH;
     P.self_first = -1;
+    P.tile_ptr = nullptr;
+    P.list = nullptr;
+    P.pool = nullptr;
+    P.list_self_blocks = 0;
+    P.U_dev = nullptr;
     if ((flags & OBEM_NBODY) && c->n_chg > 0) {
         P.sec[ns].src = c->d_chg_blk;
         P.sec[ns].nblk = ceil_div(c->n_chg, SB);
@@ -1109,6 +1184,54 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     obem_repair_kernel<<<c->sm_count, THREADS, 0, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
     c->launches += 1;
+    return OBEM_OK;
+}
+
+/* LIST-mode evaluation (obem_nn.cu): targets tgt[0..nt) ARE the point sources 0..nt-1 of the first
+ * `self_blocks` blocks of `pool` (excluded from their own sums by index); the source blocks of tile t are
+ * list[tile_ptr[t] .. tile_ptr[t+1]).  Everything, including the unit count *U_dev, is read on the device. */
+int obem_eval_list(obem_ctx* c, const float4* tgt, long long nt, float4* out, const float4* pool,
+                   const long long* tile_ptr, const int* list, const long long* U_dev, long long self_blocks, float eps,
+                   cudaStream_t st)
+{
+    if (nt <= 0) return OBEM_OK;
+    EvalParams P;
+    P.sec[0].src = pool;
+    P.sec[0].qrel = nullptr;
+    P.sec[0].nblk = 1; /* unused in LIST mode (kept non-zero: it is a divisor in the shared code) */
+    P.sec[0].npan = 0;
+    P.sec[0].stride = SBH;
+    P.sec[0].eps2 = eps * eps;
+    P.sec[0].kind = KIND_POINTS;
+    P.sec[1] = P.sec[0];
+    P.sec[1].src = nullptr;
+    P.sec[1].nblk = 0;
+    P.nblk = 1;
+    P.tgt = tgt;
+    P.nt = nt;
+    P.ntiles = ceil_div(nt, TT);
+    P.U = 0;
+    P.out = out;
+    P.ws = c->d_ws;
+    P.self_first = 0;
+    P.trk_out = nullptr;
+    P.trk_ws = c->d_trk_ws;
+    P.accumulate = 0;
+    P.tile_ptr = tile_ptr;
+    P.list = list;
+    P.pool = pool;
+    P.list_self_blocks = self_blocks;
+    P.U_dev = U_dev;
+    P.bad_count = c->d_bad_count;
+    P.bad_list = c->d_bad_list;
+    OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
+    obem_eval_kernel<KIND_POINTS, false, true><<<c->grid, THREADS, 0, st>>>(P);
+    OBEM_CUDA(c, cudaGetLastError());
+    obem_fixup_kernel<<<(unsigned)P.ntiles, THREADS, 0, st>>>(P, c->grid);
+    OBEM_CUDA(c, cudaGetLastError());
+    obem_repair_kernel<<<c->sm_count, THREADS, 0, st>>>(P);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 3;
     return OBEM_OK;
 }
 

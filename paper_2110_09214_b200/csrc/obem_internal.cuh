@@ -219,6 +219,15 @@ bool aligned4(const void* p) { return (((uintptr_t)p) & 3u) == 0; }
 int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                        float eps_nbody, cudaStream_t st, float2* trk_out = nullptr);
 
+/* obem.cu: LIST-mode evaluation kernel launch (see there).  Block layout of `pool`: OBEM_SBH float4 per block = one
+ * header (x = the weight all 256 sources share, or NaN) + 256 sources (x, y, z, w). */
+#define OBEM_SB 256
+#define OBEM_SBH 257
+#define OBEM_TT 2048
+int obem_eval_list(obem_ctx* c, const float4* tgt, long long nt, float4* out, const float4* pool,
+                   const long long* tile_ptr, const int* list, const long long* U_dev, long long self_blocks, float eps,
+                   cudaStream_t st);
+
 /* obem.cu: copy the frame origin of every panel (what panel_loop shifts the targets by) to out[0..n_pan). */
 int obem_panel_origins(obem_ctx* c, float4* out, cudaStream_t st);
 
