@@ -366,6 +366,7 @@ def run_ours(args):
         extras["next2"] = bench_next2(torch, api, ctx, wl, timed, dev, extras["nbody_only"]["s"])
         extras["next3"] = bench_next3(torch, api, ctx, wl, timed, out, extras["panels_only"]["s"])
         extras["next4"] = bench_next4(torch, api, ctx, wl, timed, dev)
+        extras["next4"]["nn_nbody"] = bench_nn(torch, api, ctx, wl, timed, out, extras["nbody_only"]["s"])
 
     # ---- roofline of the dominant kernel (obem_eval_kernel) -------------------------------------------
     sm_count = ctx.sm_count
@@ -502,6 +503,25 @@ def bench_next3(torch, api, ctx, wl, timed, out, t_panels):
     return {"panels_exact": {"s": t_ex, "overhead_vs_7_point_only": t_ex / t_panels - 1.0,
                              "first_call_with_list_build_s": t_first, "near_factor": 3.0,
                              "cell_list_entries": ctx.near_list_size, "cells": ctx.near_cells}}
+
+
+def bench_nn(torch, api, ctx, wl, timed, out, t_nbody):
+    """NN approximation of the N-body sum (paper's Table 2: 0.09 s for 1e6 particles on 1 GPU of
+    2019) on the bench workload: whole call (k-d order, leaves, lists, sums, scatter) and what it computes."""
+    n = wl.n_charges
+    peak_flops = ctx.sm_count * FP32_LANES_PER_SM * 2 * 1965.0e6 / 1e12
+    res = {}
+    for theta in (2.0, 1.0):
+        ctx.set_nn_theta(theta)
+        t = timed(lambda: ctx.eval_at_charges_nn(out=out, flags=api.NBODY))
+        units = ctx.nn_last_units()
+        inter = units * 2048 * 256
+        res["theta_%g" % theta] = {"s": t, "speedup_vs_exact_sum": t_nbody / t, "units": units,
+                                   "pair_interactions": inter, "fraction_of_exact_pairs": inter / (n * (n - 1)),
+                                   "Ginteractions_per_s_whole_call": inter / t / 1e9,
+                                   "frac_fp32_peak_whole_call": FLOP_PER_INTERACTION * inter / t / 1e12 / peak_flops}
+    ctx.set_nn_theta(2.0)
+    return res
 
 
 def bench_next4(torch, api, ctx, wl, timed, dev):

@@ -71,6 +71,10 @@ SIGNATURES = {
     "obem_set_near_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
     "obem_near_list_size": (_i64, [ctypes.c_void_p]),
     "obem_near_cells": (_i64, [ctypes.c_void_p]),
+    # NEXT-4: NN approximation of the N-body sum
+    "obem_set_nn_theta": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
+    "obem_eval_at_charges_nn": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_uint, ctypes.c_void_p]),
+    "obem_nn_last_units": (_i64, [ctypes.c_void_p, ctypes.c_void_p]),
     # NEXT-4: static field option (map + trilinear interpolation)
     "obem_field_map": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, _c_dp3, _c_dp3,
                                       _c_fp, ctypes.c_uint, ctypes.c_void_p]),
@@ -459,6 +463,27 @@ class Context:
     @property
     def near_cells(self) -> int:
         return int(_lib.obem_near_cells(self._h))
+
+    # -- NEXT-4: NN approximation of the N-body sum -----------------------------------
+    def set_nn_theta(self, theta: float = 2.0):
+        self._check(_lib.obem_set_nn_theta(self._h, float(theta)), "obem_set_nn_theta")
+
+    def eval_at_charges_nn(self, out=None, flags: int = NBODY, stream=None):
+        n = self.n_charges
+        if n < 0:
+            self._check(-2, "obem_eval_at_charges_nn")
+        if out is None:
+            out = self._new((n, 4))
+        elif n:
+            _dev_f32(out, "out", (4,))
+            if out.shape[0] != n:
+                raise ValueError("out must be [n_charges, 4]")
+        self._check(_lib.obem_eval_at_charges_nn(self._h, out.data_ptr() if n else None, int(flags),
+                                                 _stream_ptr(stream)), "obem_eval_at_charges_nn")
+        return out
+
+    def nn_last_units(self, stream=None) -> int:
+        return int(_lib.obem_nn_last_units(self._h, _stream_ptr(stream)))
 
     # -- NEXT-4: static field option ------------------------------------------------------
     def field_map(self, shape, origin, spacing, flags: int = PANELS, out=None, stream=None):

@@ -1316,6 +1316,7 @@ int obem_destroy(obem_ctx* c)
     if (c->d_step_field) cudaFree(c->d_step_field);
     if (c->d_map_pts) cudaFree(c->d_map_pts);
     obem_near_free(c);
+    obem_nn_free(c);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_trk_ws) cudaFree(c->d_trk_ws);
     if (c->d_trk) cudaFree(c->d_trk);

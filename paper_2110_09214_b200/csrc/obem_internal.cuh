@@ -112,6 +112,28 @@ inline long long ceil_div(long long a, long long b) { return (a + b - 1) / b; }
 
 } /* namespace */
 
+/* obem_nn.cu: buffers of the NN approximation (all library-owned, grown on demand) */
+struct obem_nn_state {
+    float theta = 2.0f;
+    int* perm[2] = {nullptr, nullptr};
+    unsigned long long* key[2] = {nullptr, nullptr};
+    size_t perm_cap[2] = {0, 0}, key_cap[2] = {0, 0};
+    unsigned* seg = nullptr;         /* [2][n_leaf][3] ordered min / max coordinates of the segments of a level */
+    float4* sorted = nullptr;        /* [n_leaf * 256] the charges in k-d order (padded): the targets           */
+    float4* pool = nullptr;          /* [(n_leaf + n_group * far_blocks)][OBEM_SBH] leaf blocks, then far blocks */
+    float* leafbox = nullptr;        /* [n_leaf][6] */
+    float4* pseudo = nullptr;        /* [n_leaf][2] centre of charge of the positive / negative members         */
+    long long* cnt = nullptr;        /* [n_group] units of each tile */
+    long long* tile_ptr = nullptr;   /* [n_group + 1] + the unit count U */
+    int* list = nullptr;
+    float4* out_sorted = nullptr;
+    void* tmp = nullptr;             /* radix-sort workspace */
+    float4* pan = nullptr;           /* panel part when the flags ask for it */
+    size_t seg_cap = 0, sorted_cap = 0, pool_cap = 0, leafbox_cap = 0, pseudo_cap = 0, cnt_cap = 0, tile_ptr_cap = 0,
+           list_cap = 0, out_sorted_cap = 0, tmp_cap = 0, pan_cap = 0;
+    long long last_n = 0;
+};
+
 struct obem_ctx {
     int device = 0;
     int sm_count = 0;
@@ -173,6 +195,7 @@ struct obem_ctx {
     float4* d_exact_tmp = nullptr;    /* [nt] panel part of an N-body + exact-panels evaluation */
     long long exact_tmp_cap = 0;
     long long near_entries = -1; /* (cell, panel) entries of the current lists; -1 before the first build */
+    obem_nn_state nn;
     /* obem_map.cu */
     float4* d_map_pts = nullptr; /* node coordinates of the last obem_field_map */
     size_t map_pts_cap = 0;      /* bytes */
@@ -242,5 +265,7 @@ int obem_near_correct(obem_ctx* c, const float4* tgt, long long nt, float4* out,
 int obem_eval_exact(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                     float eps_nbody, cudaStream_t st, float2* trk_out);
 void obem_near_free(obem_ctx* c);
+
+void obem_nn_free(obem_ctx* c);
 
 #endif /* OBEM_INTERNAL_CUH */

@@ -1,0 +1,435 @@
+/*
+ * obem_nn.cu -- the nearest-neighbour (NN) approximation of the N-body sum (
+ * PAPER.md:279-296, section 3.2.4): "evaluating the exact Coulombian field following (3.8) for each of the closest
+ * particles to the particle of interest while the field from the particles further away is approximated by their
+ * centre of charges with a barycentric method."  The paper says no more; the algorithm is DESIGN.md reading A19:
+ *
+ *   1. k-d partition with equal-count leaves: level by level, every segment of more than 256 charges is sorted
+ *      (stably) along the longest axis of its bounding box and cut at a multiple of 256 -- one radix sort per level
+ *      over the whole array with key = (segment start, coordinate).  A leaf = 256 charges = one source block of the
+ *      evaluation kernel; a target group = 8 consecutive leaves = one 2048-target tile.
+ *   2. Per leaf: bounding box and two pseudo-particles (the centres of charge of its positive and of its negative
+ *      members).
+ *   3. Per (tile, leaf): FAR iff theta^2 dist2(box_tile, box_leaf) > diag2(box_leaf), decided in fp64 with
+ *      individually rounded operations (the oracle takes the same decisions bit for bit).
+ *   4. Tile t's source list = its near leaves (the charges themselves, exact Eq 3.8, self excluded by index) + its
+ *      own copy of all pseudo-particles with the near leaves' ones blanked -- run by the LIST instantiation of the
+ *      hot path's evaluation kernel (obem.cu), stream-K over all (tile, block) units.
+ *   5. Results are scattered back to the input order.
+ *
+ * Every step is enqueued on the caller's stream; nothing is read back to the host (all sizes follow from n).
+ * Part of libobem.so; shares nothing with oracle/.
+ */
+#include <cub/device/device_radix_sort.cuh>
+
+#include "obem_internal.cuh"
+
+namespace {
+
+typedef unsigned long long u64k;
+constexpr int LEAF = OBEM_SB;        /* 256 */
+constexpr int GROUP = OBEM_TT;       /* 2048 */
+constexpr int LPG = GROUP / LEAF;    /* leaves per group */
+constexpr int PPB_FAR = LEAF / 2;    /* leaves whose two pseudo-particles fill one far block */
+constexpr float NN_PAD_FAR = 1.0e15f;
+
+__host__ __device__ __forceinline__ long long nn_split(long long a, long long b)
+{
+    const long long leaves = (b - a + LEAF - 1) / LEAF;
+    return a + (long long)LEAF * ((leaves + 1) / 2);
+}
+/* segment [a, b) that holds position i after `level` rounds of cuts */
+__device__ __forceinline__ void nn_segment(long long n, long long i, int level, long long& a, long long& b)
+{
+    a = 0, b = n;
+    for (int t = 0; t < level && b - a > LEAF; ++t) {
+        const long long m = nn_split(a, b);
+        if (i < m) b = m;
+        else a = m;
+    }
+}
+/* fp32 bits -> unsigned whose order is the IEEE total order of the floats */
+__device__ __forceinline__ unsigned nn_ordered(float f)
+{
+    const unsigned u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float nn_unordered(unsigned k)
+{
+    return __uint_as_float((k & 0x80000000u) ? (k & 0x7fffffffu) : ~k);
+}
+
+__global__ void nn_iota_kernel(int* __restrict__ perm, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) perm[i] = (int)i;
+}
+
+/* segmin[s][0..2], segmax[s][0..2] = min, max of the ordered coordinates of segment s = (segment start)/256
+ * (initialised to 0xffffffff and 0 by the caller).  min / max
+ * are order independent, so the atomics do not make the result depend on scheduling. */
+__global__ void nn_segbox_kernel(const float4* __restrict__ x, const int* __restrict__ perm, long long n, int level,
+                                 unsigned* __restrict__ segmin, unsigned* __restrict__ segmax)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    long long a, b;
+    nn_segment(n, i, level, a, b);
+    if (b - a <= LEAF) return; /* final: not sorted again */
+    const float4 p = x[perm[i]];
+    const unsigned k[3] = {nn_ordered(p.x), nn_ordered(p.y), nn_ordered(p.z)};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        atomicMin(segmin + (a / LEAF) * 3 + d, k[d]);
+        atomicMax(segmax + (a / LEAF) * 3 + d, k[d]);
+    }
+}
+
+__global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restrict__ perm, long long n, int level,
+                              const unsigned* __restrict__ segmin, const unsigned* __restrict__ segmax,
+                              u64k* __restrict__ keys)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    long long a, b;
+    nn_segment(n, i, level, a, b);
+    unsigned low;
+    if (b - a <= LEAF) {
+        low = (unsigned)(i - a); /* keep the order of a final segment */
+    } else {
+        double ext[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d)
+            ext[d] = (double)nn_unordered(segmax[(a / LEAF) * 3 + d]) - (double)nn_unordered(segmin[(a / LEAF) * 3 + d]);
+        int ax = 0; /* the first axis of the largest extent */
+        if (ext[1] > ext[ax]) ax = 1;
+        if (ext[2] > ext[ax]) ax = 2;
+        const float4 p = x[perm[i]];
+        low = nn_ordered(ax == 0 ? p.x : (ax == 1 ? p.y : p.z));
+    }
+    keys[i] = ((u64k)a << 32) | (u64k)low;
+}
+
+/* one CTA per leaf: sorted copy (plain, padded) + blocked copy with header + bounding box + the two pseudo-particles */
+__global__ void __launch_bounds__(LEAF) nn_leaf_kernel(const float4* __restrict__ x, const int* __restrict__ perm,
+                                                        long long n, float4* __restrict__ sorted,
+                                                        float4* __restrict__ pool, float* __restrict__ leafbox,
+                                                        float4* __restrict__ pseudo)
+{
+    __shared__ double red[8][LEAF / 32];
+    __shared__ float fred[6][LEAF / 32];
+    const long long l = blockIdx.x, i = l * LEAF + threadIdx.x;
+    const bool valid = i < n;
+    const float4 v = valid ? x[perm[i]] : make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
+    sorted[i] = v;
+    pool[l * OBEM_SBH + 1 + threadIdx.x] = v;
+    const float w0 = x[perm[l * LEAF]].w;
+    const int uniform = __syncthreads_and(v.w == w0);
+    if (threadIdx.x == 0) pool[l * OBEM_SBH] = make_float4(uniform ? w0 : __int_as_float(0x7fc00000), 0.f, 0.f, 0.f);
+    /* box over the valid members, charge and first moment of the positive and of the negative members */
+    const float big = __int_as_float(0x7f800000);
+    float lo[3] = {valid ? v.x : big, valid ? v.y : big, valid ? v.z : big};
+    float hi[3] = {valid ? v.x : -big, valid ? v.y : -big, valid ? v.z : -big};
+    const double q = (double)v.w;
+    double m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (valid && v.w > 0.f) m[0] = q, m[1] = q * v.x, m[2] = q * v.y, m[3] = q * v.z;
+    if (valid && v.w < 0.f) m[4] = q, m[5] = q * v.x, m[6] = q * v.y, m[7] = q * v.z;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            lo[d] = fminf(lo[d], __shfl_xor_sync(0xffffffffu, lo[d], o));
+            hi[d] = fmaxf(hi[d], __shfl_xor_sync(0xffffffffu, hi[d], o));
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) m[k] += __shfl_xor_sync(0xffffffffu, m[k], o);
+    }
+    if (lane == 0) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) fred[d][w] = lo[d], fred[3 + d][w] = hi[d];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) red[k][w] = m[k];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int ww = 1; ww < LEAF / 32; ++ww) {
+            for (int d = 0; d < 3; ++d) {
+                fred[d][0] = fminf(fred[d][0], fred[d][ww]);
+                fred[3 + d][0] = fmaxf(fred[3 + d][0], fred[3 + d][ww]);
+            }
+            for (int k = 0; k < 8; ++k) red[k][0] += red[k][ww];
+        }
+        for (int d = 0; d < 6; ++d) leafbox[l * 6 + d] = fred[d][0];
+        for (int h = 0; h < 2; ++h) {
+            const double Q = red[4 * h][0];
+            pseudo[l * 2 + h] = (Q != 0.0) ? make_float4((float)(red[4 * h + 1][0] / Q), (float)(red[4 * h + 2][0] / Q),
+                                                         (float)(red[4 * h + 3][0] / Q), (float)Q)
+                                           : make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
+        }
+    }
+}
+
+/* FAR iff theta^2 * dist2(box_g, box_l) > diag2(box_l); every operation rounded on its own (no contraction), x, y, z
+ * in this order -- the oracle forms the same expression in numpy */
+__device__ __forceinline__ bool nn_is_far(const float (&g)[6], const float* __restrict__ lb, double theta2)
+{
+    double dist2 = 0.0, diag2 = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const double a = (double)lb[d] - (double)g[3 + d], b = (double)g[d] - (double)lb[3 + d];
+        const double gap = fmax(0.0, fmax(a, b));
+        const double side = (double)lb[3 + d] - (double)lb[d];
+        const double g2 = __dmul_rn(gap, gap), s2 = __dmul_rn(side, side);
+        dist2 = (d == 0) ? g2 : __dadd_rn(dist2, g2);
+        diag2 = (d == 0) ? s2 : __dadd_rn(diag2, s2);
+    }
+    return __dmul_rn(theta2, dist2) > diag2;
+}
+
+__device__ __forceinline__ void nn_group_box(const float* __restrict__ leafbox, long long g, long long n_leaf, float (&gb)[6])
+{
+    const float big = __int_as_float(0x7f800000);
+    for (int d = 0; d < 3; ++d) gb[d] = big, gb[3 + d] = -big;
+    for (long long l = g * LPG; l < (g + 1) * LPG && l < n_leaf; ++l)
+        for (int d = 0; d < 3; ++d) {
+            gb[d] = fminf(gb[d], leafbox[l * 6 + d]);
+            gb[3 + d] = fmaxf(gb[3 + d], leafbox[l * 6 + 3 + d]);
+        }
+}
+
+/* one CTA per group.  FILL = false: cnt[g] = (near leaves) + (far blocks).  FILL = true: write the group's list
+ * (near leaf blocks in ascending order, then its far blocks) and its far blocks (all pseudo-particles, the near
+ * leaves' ones blanked). */
+template <bool FILL>
+__global__ void __launch_bounds__(256) nn_lists_kernel(const float* __restrict__ leafbox, const float4* __restrict__ pseudo,
+                                                       long long n_leaf, long long far_blocks, double theta2,
+                                                       long long* __restrict__ cnt, const long long* __restrict__ tile_ptr,
+                                                       int* __restrict__ list, float4* __restrict__ pool)
+{
+    __shared__ int wsum[8];
+    __shared__ int base_sh;
+    const long long g = blockIdx.x;
+    float gb[6];
+    nn_group_box(leafbox, g, n_leaf, gb);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) base_sh = 0;
+    __syncthreads();
+    float4* far = FILL ? pool + (n_leaf + g * far_blocks) * OBEM_SBH : nullptr;
+    int* out = FILL ? list + tile_ptr[g] : nullptr;
+    const long long l_end = far_blocks * PPB_FAR; /* leaves incl. the padding of the last far block */
+    for (long long l0 = 0; l0 < l_end; l0 += 256) {
+        const long long l = l0 + threadIdx.x;
+        const bool real = l < n_leaf;
+        const bool near = real && !nn_is_far(gb, leafbox + l * 6, theta2);
+        const unsigned bal = __ballot_sync(0xffffffffu, near);
+        if (lane == 0) wsum[w] = __popc(bal);
+        __syncthreads();
+        int before = base_sh, total = 0;
+        for (int ww = 0; ww < 8; ++ww) {
+            if (ww < w) before += wsum[ww];
+            total += wsum[ww];
+        }
+        if (FILL) {
+            if (near) out[before + __popc(bal & ((1u << lane) - 1u))] = (int)l;
+            if (l < l_end) {
+                const float4 blank = make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
+                float4* dst = far + (l / PPB_FAR) * OBEM_SBH + 1 + 2 * (l % PPB_FAR);
+                dst[0] = (real && !near) ? pseudo[l * 2] : blank;
+                dst[1] = (real && !near) ? pseudo[l * 2 + 1] : blank;
+                if (l % PPB_FAR == 0) dst[-1] = make_float4(__int_as_float(0x7fc00000), 0.f, 0.f, 0.f); /* header */
+            }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) base_sh += total;
+        __syncthreads();
+    }
+    if (FILL) {
+        for (long long k = threadIdx.x; k < far_blocks; k += 256) out[base_sh + k] = (int)(n_leaf + g * far_blocks + k);
+    } else if (threadIdx.x == 0) {
+        cnt[g] = base_sh + far_blocks;
+    }
+}
+
+/* tile_ptr = exclusive prefix sum of cnt (n_group <= a few thousand: one thread), U = the total */
+__global__ void nn_scan_kernel(const long long* __restrict__ cnt, long long n_group, long long* __restrict__ tile_ptr,
+                               long long* __restrict__ U)
+{
+    if (blockIdx.x || threadIdx.x) return;
+    long long s = 0;
+    for (long long g = 0; g < n_group; ++g) {
+        tile_ptr[g] = s;
+        s += cnt[g];
+    }
+    tile_ptr[n_group] = s;
+    *U = s;
+}
+
+__global__ void nn_scatter_kernel(const float4* __restrict__ sorted_out, const int* __restrict__ perm, long long n,
+                                  float4* __restrict__ out)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[perm[i]] = sorted_out[i];
+}
+
+__global__ void nn_add_kernel(float4* __restrict__ out, const float4* __restrict__ b, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = out[i], q = b[i];
+    out[i] = make_float4(p.x + q.x, p.y + q.y, p.z + q.z, p.w + q.w);
+}
+
+} /* namespace */
+
+namespace {
+
+template <typename T>
+int nn_grow(obem_ctx* c, T*& p, size_t& cap, size_t count)
+{
+    const size_t bytes = count * sizeof(T);
+    if (bytes <= cap) return OBEM_OK;
+    if (p) cudaFree(p);
+    p = nullptr, cap = 0;
+    OBEM_CUDA(c, cudaMalloc(&p, bytes));
+    cap = bytes;
+    return OBEM_OK;
+}
+
+} /* namespace */
+
+void obem_nn_free(obem_ctx* c)
+{
+    void* ptrs[] = {c->nn.perm[0], c->nn.perm[1], c->nn.key[0], c->nn.key[1], c->nn.seg, c->nn.sorted, c->nn.pool,
+                    c->nn.leafbox, c->nn.pseudo, c->nn.cnt, c->nn.tile_ptr, c->nn.list, c->nn.out_sorted, c->nn.tmp,
+                    c->nn.pan};
+    for (void* p : ptrs)
+        if (p) cudaFree(p);
+}
+
+extern "C" {
+
+int obem_set_nn_theta(obem_ctx* c, float theta)
+{
+    if (!c || !(theta >= 0.f) || !isfinite(theta)) return OBEM_EINVAL;
+    c->nn.theta = theta;
+    return OBEM_OK;
+}
+
+int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cuda_stream)
+{
+    if (!c) return OBEM_EINVAL;
+    if (flags & ~(OBEM_NBODY | OBEM_PANELS | OBEM_PANELS_EXACT)) return OBEM_EINVAL;
+    if (!(flags & OBEM_NBODY)) return OBEM_EINVAL;
+    if ((flags & OBEM_PANELS_EXACT) && !(flags & OBEM_PANELS)) return OBEM_EINVAL;
+    if (c->n_chg < 0) return OBEM_ESTATE;
+    if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
+    const long long n = c->n_chg;
+    if (n == 0) return OBEM_OK;
+    if (!d_out || !aligned16(d_out)) return OBEM_EINVAL;
+    if (n > 0x7fffffffLL - GROUP) return OBEM_EINVAL;
+    DeviceGuard dg(c->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    obem_nn_state& S = c->nn;
+    const long long n_leaf = ceil_div(n, LEAF), n_group = ceil_div(n, GROUP);
+    const long long far_blocks = ceil_div(n_leaf, PPB_FAR);
+    int levels = 0;
+    while ((1LL << levels) < n_leaf) ++levels;
+    int nbits = 1;
+    while ((1LL << nbits) <= n) ++nbits;
+
+    int rc = OBEM_OK;
+    for (int k = 0; k < 2 && rc == OBEM_OK; ++k) {
+        rc = nn_grow(c, S.perm[k], S.perm_cap[k], (size_t)n);
+        if (rc == OBEM_OK) rc = nn_grow(c, S.key[k], S.key_cap[k], (size_t)n);
+    }
+    if (rc == OBEM_OK) rc = nn_grow(c, S.seg, S.seg_cap, (size_t)n_leaf * 6);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.sorted, S.sorted_cap, (size_t)n_leaf * LEAF);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.pool, S.pool_cap, (size_t)(n_leaf + n_group * far_blocks) * OBEM_SBH);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.leafbox, S.leafbox_cap, (size_t)n_leaf * 6);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.pseudo, S.pseudo_cap, (size_t)n_leaf * 2);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.cnt, S.cnt_cap, (size_t)n_group);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.tile_ptr, S.tile_ptr_cap, (size_t)n_group + 2); /* [n_group + 1] + U */
+    if (rc == OBEM_OK) rc = nn_grow(c, S.list, S.list_cap, (size_t)n_group * (size_t)(n_leaf + far_blocks));
+    if (rc == OBEM_OK) rc = nn_grow(c, S.out_sorted, S.out_sorted_cap, (size_t)n);
+    if (rc != OBEM_OK) return rc;
+    size_t tmp_bytes = 0;
+    OBEM_CUDA(c, cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, S.key[0], S.key[1], S.perm[0], S.perm[1], (int)n, 0,
+                                                 32 + nbits, st));
+    {
+        unsigned char* t = (unsigned char*)S.tmp;
+        rc = nn_grow(c, t, S.tmp_cap, tmp_bytes);
+        S.tmp = t;
+        if (rc != OBEM_OK) return rc;
+    }
+
+    const unsigned gn = (unsigned)ceil_div(n, 256);
+    /* 1. k-d order */
+    nn_iota_kernel<<<gn, 256, 0, st>>>(S.perm[0], n);
+    OBEM_CUDA(c, cudaGetLastError());
+    int cur = 0;
+    unsigned* segmin = S.seg;
+    unsigned* segmax = S.seg + n_leaf * 3;
+    for (int level = 0; level < levels; ++level) {
+        OBEM_CUDA(c, cudaMemsetAsync(segmin, 0xff, (size_t)n_leaf * 3 * sizeof(unsigned), st));
+        OBEM_CUDA(c, cudaMemsetAsync(segmax, 0x00, (size_t)n_leaf * 3 * sizeof(unsigned), st));
+        nn_segbox_kernel<<<gn, 256, 0, st>>>(c->d_chg, S.perm[cur], n, level, segmin, segmax);
+        OBEM_CUDA(c, cudaGetLastError());
+        nn_key_kernel<<<gn, 256, 0, st>>>(c->d_chg, S.perm[cur], n, level, segmin, segmax, S.key[cur]);
+        OBEM_CUDA(c, cudaGetLastError());
+        OBEM_CUDA(c, cub::DeviceRadixSort::SortPairs(S.tmp, tmp_bytes, S.key[cur], S.key[cur ^ 1], S.perm[cur],
+                                                     S.perm[cur ^ 1], (int)n, 0, 32 + nbits, st));
+        cur ^= 1;
+        c->launches += 3;
+    }
+    const int* perm = S.perm[cur];
+    /* 2. leaves */
+    nn_leaf_kernel<<<(unsigned)n_leaf, LEAF, 0, st>>>(c->d_chg, perm, n, S.sorted, S.pool, S.leafbox, S.pseudo);
+    OBEM_CUDA(c, cudaGetLastError());
+    /* 3. + 4. per-tile lists and far blocks */
+    const double theta2 = (double)S.theta * (double)S.theta;
+    long long* U_dev = S.tile_ptr + n_group + 1;
+    nn_lists_kernel<false><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, n_leaf, far_blocks, theta2, S.cnt,
+                                                              nullptr, nullptr, nullptr);
+    OBEM_CUDA(c, cudaGetLastError());
+    nn_scan_kernel<<<1, 32, 0, st>>>(S.cnt, n_group, S.tile_ptr, U_dev);
+    OBEM_CUDA(c, cudaGetLastError());
+    nn_lists_kernel<true><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, n_leaf, far_blocks, theta2, S.cnt,
+                                                             S.tile_ptr, S.list, S.pool);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 5;
+    /* 5. the sums, in sorted order, then back to the input order */
+    rc = obem_eval_list(c, S.sorted, n, S.out_sorted, S.pool, S.tile_ptr, S.list, U_dev, n_leaf, c->eps_pp, st);
+    if (rc != OBEM_OK) return rc;
+    nn_scatter_kernel<<<gn, 256, 0, st>>>(S.out_sorted, perm, n, (float4*)d_out);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 1;
+    S.last_n = n;
+    if (flags & OBEM_PANELS) {
+        rc = nn_grow(c, S.pan, S.pan_cap, (size_t)n);
+        if (rc != OBEM_OK) return rc;
+        rc = obem_eval_internal(c, c->d_chg, n, S.pan, flags & ~OBEM_NBODY, -1, c->eps_pp, st);
+        if (rc != OBEM_OK) return rc;
+        nn_add_kernel<<<gn, 256, 0, st>>>((float4*)d_out, S.pan, n);
+        OBEM_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
+    return OBEM_OK;
+}
+
+int64_t obem_nn_last_units(obem_ctx* c, void* cuda_stream)
+{
+    if (!c || c->nn.last_n <= 0 || !c->nn.tile_ptr) return -1;
+    DeviceGuard dg(c->device);
+    long long U = -1;
+    const long long n_group = ceil_div(c->nn.last_n, GROUP);
+    if (cudaMemcpyAsync(&U, c->nn.tile_ptr + n_group + 1, sizeof(U), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream) !=
+            cudaSuccess ||
+        cudaStreamSynchronize((cudaStream_t)cuda_stream) != cudaSuccess) {
+        cudaGetLastError();
+        return -1;
+    }
+    return U;
+}
+
+} /* extern "C" */
