@@ -68,20 +68,71 @@ __global__ void nn_iota_kernel(int* __restrict__ perm, long long n)
 /* segmin[s][0..2], segmax[s][0..2] = min, max of the ordered coordinates of segment s = (segment start)/256
  * (initialised to 0xffffffff and 0 by the caller).  min / max
  * are order independent, so the atomics do not make the result depend on scheduling. */
-__global__ void nn_segbox_kernel(const float4* __restrict__ x, const int* __restrict__ perm, long long n, int level,
-                                 unsigned* __restrict__ segmin, unsigned* __restrict__ segmax)
+__global__ void __launch_bounds__(256) nn_segbox_kernel(const float4* __restrict__ x, const int* __restrict__ perm,
+                                                        long long n, int level, unsigned* __restrict__ segmin,
+                                                        unsigned* __restrict__ segmax)
 {
+    __shared__ unsigned sh[6][8];
+    __shared__ long long sh_a[8];
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    long long a, b;
-    nn_segment(n, i, level, a, b);
-    if (b - a <= LEAF) return; /* final: not sorted again */
-    const float4 p = x[perm[i]];
-    const unsigned k[3] = {nn_ordered(p.x), nn_ordered(p.y), nn_ordered(p.z)};
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    long long a = -1, b = -1;
+    unsigned k[6] = {0xffffffffu, 0xffffffffu, 0xffffffffu, 0u, 0u, 0u};
+    if (i < n) {
+        nn_segment(n, i, level, a, b);
+        if (b - a <= LEAF) a = -1; /* final: not sorted again */
+        else {
+            const float4 p = x[perm[i]];
+            k[0] = k[3] = nn_ordered(p.x), k[1] = k[4] = nn_ordered(p.y), k[2] = k[5] = nn_ordered(p.z);
+        }
+    }
+    /* a warp that lies inside one segment (almost all do) reduces first; so does a block of such warps */
+    const long long a0 = __shfl_sync(0xffffffffu, a, 0);
+    const bool warp_same = __all_sync(0xffffffffu, a == a0);
+    if (!warp_same) {
+        if (a >= 0) {
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        atomicMin(segmin + (a / LEAF) * 3 + d, k[d]);
-        atomicMax(segmax + (a / LEAF) * 3 + d, k[d]);
+            for (int d = 0; d < 3; ++d) {
+                atomicMin(segmin + (a / LEAF) * 3 + d, k[d]);
+                atomicMax(segmax + (a / LEAF) * 3 + d, k[3 + d]);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            k[d] = __reduce_min_sync(0xffffffffu, k[d]);
+            k[3 + d] = __reduce_max_sync(0xffffffffu, k[3 + d]);
+        }
+    }
+    if (lane == 0) {
+        sh_a[w] = warp_same ? a0 : -2; /* -2: this warp has already written */
+#pragma unroll
+        for (int d = 0; d < 6; ++d) sh[d][w] = k[d];
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        /* merge runs of consecutive warps of the same segment, one atomic per run and component */
+        int w0 = 0;
+        while (w0 < 8) {
+            const long long sa = sh_a[w0];
+            int w1 = w0 + 1;
+            unsigned m[6];
+            for (int d = 0; d < 6; ++d) m[d] = sh[d][w0];
+            while (w1 < 8 && sh_a[w1] == sa) {
+                for (int d = 0; d < 3; ++d) {
+                    m[d] = min(m[d], sh[d][w1]);
+                    m[3 + d] = max(m[3 + d], sh[3 + d][w1]);
+                }
+                ++w1;
+            }
+            if (sa >= 0) {
+                for (int d = 0; d < 3; ++d) {
+                    atomicMin(segmin + (sa / LEAF) * 3 + d, m[d]);
+                    atomicMax(segmax + (sa / LEAF) * 3 + d, m[3 + d]);
+                }
+            }
+            w0 = w1;
+        }
     }
 }
 
