@@ -249,6 +249,25 @@ int obem_set_near_field(obem_ctx* c, float near_factor);
 int64_t obem_near_list_size(const obem_ctx* c);
 int64_t obem_near_cells(const obem_ctx* c);
 
+/* Polygonal cells ("flat polygonal cells (triangles, quadrangles, etc.)", one constant sigma
+ * each).  d_verts4 [n_cells][4][3] fp32, d_nvert [n_cells] int32 = 3 or 4 (NULL: all 4; for 3 the 4th vertex is
+ * ignored), d_sigma [n_cells].  A flat quadrilateral (v0, v1, v2, v3), vertices in order around the cell, is stored
+ * as the triangles (v0, v1, v2), (v0, v2, v3) with the same sigma; a triangle cell as itself plus a zero-area one.
+ * Afterwards the context holds 2 n_cells panels (obem_n_panels, obem_influence_on_panels ... count triangles);
+ * obem_set_sigma_cells updates sigma per CELL. */
+int obem_set_panels_cells(obem_ctx* c, const float* d_verts4, const int32_t* d_nvert, const float* d_sigma,
+                          int64_t n_cells, void* cuda_stream);
+int obem_set_sigma_cells(obem_ctx* c, const float* d_sigma, int64_t n_cells, void* cuda_stream);
+
+/* Symmetry planes ("up to three symmetry planes can also be included").  n_planes in 0..3 (0 removes
+ * them); plane k is x_{h_axis[k]} = h_coord[k] [m] (axis 0, 1, 2 = x, y, z; at most one plane per axis) with parity
+ * h_parity[k] = +1 (the mirror image of every source carries the same charge) or -1 (the opposite charge: a
+ * grounded plane).  HOST arrays.  From then on every evaluate call (and stepper, influence, field map) adds the
+ * 2^n - 1 image copies of ALL sources the flags select: each image is evaluated as reflected targets on the original
+ * sources, E_image(r) = s M E(M r), so the cost is 2^n evaluations and nothing is duplicated in memory.  The image of
+ * charge i acts on charge i.  Not combined with obem_eval_at_charges_nn (OBEM_EINVAL). */
+int obem_set_symmetry(obem_ctx* c, int n_planes, const int* h_axis, const double* h_coord, const int* h_parity);
+
 /* ----------------------------------------------------------------------------------------------------------
  * NEXT-4: the static field option, section 3.2.1: "the field components are computed only once at
  * some predefined spatial coordinates located on a uniform 3D grid map ... During the transport, the field

@@ -71,6 +71,10 @@ SIGNATURES = {
     "obem_set_near_field": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
     "obem_near_list_size": (_i64, [ctypes.c_void_p]),
     "obem_near_cells": (_i64, [ctypes.c_void_p]),
+    "obem_set_panels_cells": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _i64, ctypes.c_void_p]),
+    "obem_set_sigma_cells": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, ctypes.c_void_p]),
+    "obem_set_symmetry": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_int), _c_dp3,
+                                         ctypes.POINTER(ctypes.c_int)]),
     # NEXT-4: NN approximation of the N-body sum
     "obem_set_nn_theta": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_float]),
     "obem_eval_at_charges_nn": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_uint, ctypes.c_void_p]),
@@ -463,6 +467,37 @@ class Context:
     @property
     def near_cells(self) -> int:
         return int(_lib.obem_near_cells(self._h))
+
+    def set_panels_cells(self, verts4, sigma, nvert=None, stream=None):
+        """verts4 [Nc,4,3] float32, sigma [Nc] float32, nvert [Nc] int32 (3 or 4; None = all quadrilaterals)."""
+        torch = _torch()
+        nc = int(sigma.shape[0])
+        if nc:
+            _dev_f32(verts4, "verts4", (4, 3)), _dev_f32(sigma, "sigma")
+            if verts4.shape[0] != nc:
+                raise ValueError("verts4 and sigma disagree on the number of cells")
+            if nvert is not None and (not nvert.is_cuda or nvert.dtype != torch.int32 or nvert.shape != (nc,)):
+                raise TypeError("nvert must be an int32 CUDA tensor of shape [n_cells]")
+        self._check(_lib.obem_set_panels_cells(self._h, verts4.data_ptr() if nc else None,
+                                               nvert.data_ptr() if (nc and nvert is not None) else None,
+                                               sigma.data_ptr() if nc else None, nc, _stream_ptr(stream)),
+                    "obem_set_panels_cells")
+
+    def set_sigma_cells(self, sigma, stream=None):
+        nc = int(sigma.shape[0])
+        if nc:
+            _dev_f32(sigma, "sigma")
+        self._check(_lib.obem_set_sigma_cells(self._h, sigma.data_ptr() if nc else None, nc, _stream_ptr(stream)),
+                    "obem_set_sigma_cells")
+
+    def set_symmetry(self, planes=()):
+        """planes: iterable of (axis 0|1|2, coordinate [m], parity +1|-1); at most one per axis; () removes them."""
+        planes = list(planes)
+        n = len(planes)
+        ax = (ctypes.c_int * max(n, 1))(*[int(p[0]) for p in planes])
+        co = (ctypes.c_double * max(n, 1))(*[float(p[1]) for p in planes])
+        pa = (ctypes.c_int * max(n, 1))(*[int(p[2]) for p in planes])
+        self._check(_lib.obem_set_symmetry(self._h, n, ax, co, pa), "obem_set_symmetry")
 
     # -- NEXT-4: NN approximation of the N-body sum (PAPER.md:279-296) -----------------------------------
     def set_nn_theta(self, theta: float = 2.0):

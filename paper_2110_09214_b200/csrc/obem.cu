@@ -1103,6 +1103,8 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     if ((flags & OBEM_NBODY) && c->n_chg < 0) return OBEM_ESTATE;
     if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
     if (nt == 0) return OBEM_OK;
+    /* NEXT-3: symmetry planes = image sources, evaluated as reflected targets (obem_geom.cu) */
+    if (c->sym_n > 0 && !c->sym_busy) return obem_eval_symmetric(c, tgt, nt, out, flags, self_first, eps_nbody, st, trk_out);
     /* NEXT-3: exact integrals for the panels near each target (obem_near.cu) */
     if ((flags & OBEM_PANELS_EXACT) && c->n_pan > 0)
         return obem_eval_exact(c, tgt, nt, out, flags & ~OBEM_PANELS_EXACT, self_first, eps_nbody, st, trk_out);
@@ -1319,6 +1321,7 @@ int obem_destroy(obem_ctx* c)
     if (c->d_map_pts) cudaFree(c->d_map_pts);
     obem_near_free(c);
     obem_nn_free(c);
+    obem_geom_free(c);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_trk_ws) cudaFree(c->d_trk_ws);
     if (c->d_trk) cudaFree(c->d_trk);

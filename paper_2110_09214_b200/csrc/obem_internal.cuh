@@ -196,6 +196,16 @@ struct obem_ctx {
     long long exact_tmp_cap = 0;
     long long near_entries = -1; /* (cell, panel) entries of the current lists; -1 before the first build */
     obem_nn_state nn;
+    /* obem_geom.cu: symmetry planes and polygonal cells */
+    int sym_n = 0, sym_axis[3] = {0, 0, 0}, sym_sign[3] = {1, 1, 1};
+    double sym_coord[3] = {0, 0, 0};
+    int sym_busy = 0;             /* inside obem_eval_symmetric: its own calls evaluate plainly */
+    float4* d_sym_pts = nullptr;  /* reflected targets of one image */
+    float4* d_sym_out = nullptr;  /* that image's field */
+    size_t sym_pts_cap = 0, sym_out_cap = 0;
+    float* d_cell_tri = nullptr;  /* [2 n_cells][3][3] triangles of the polygonal cells */
+    float* d_cell_sig = nullptr;  /* [2 n_cells] */
+    size_t cell_tri_cap = 0, cell_sig_cap = 0;
     /* obem_map.cu */
     float4* d_map_pts = nullptr; /* node coordinates of the last obem_field_map */
     size_t map_pts_cap = 0;      /* bytes */
@@ -267,5 +277,9 @@ int obem_eval_exact(obem_ctx* c, const float4* tgt, long long nt, float4* out, u
 void obem_near_free(obem_ctx* c);
 
 void obem_nn_free(obem_ctx* c);
+/* obem_geom.cu */
+int obem_eval_symmetric(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
+                        float eps_nbody, cudaStream_t st, float2* trk_out);
+void obem_geom_free(obem_ctx* c);
 
 #endif /* OBEM_INTERNAL_CUH */

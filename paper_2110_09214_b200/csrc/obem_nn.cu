@@ -375,6 +375,7 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     if ((flags & OBEM_PANELS_EXACT) && !(flags & OBEM_PANELS)) return OBEM_EINVAL;
     if (c->n_chg < 0) return OBEM_ESTATE;
     if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
+    if (c->sym_n > 0) return OBEM_EINVAL; /* the lists hold no image leaves */
     const long long n = c->n_chg;
     if (n == 0) return OBEM_OK;
     if (!d_out || !aligned16(d_out)) return OBEM_EINVAL;
