@@ -378,7 +378,8 @@ def run_ours(args):
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
         "traffic": TRAFFIC_BYTES_PER_LAUNCH if world == 1 and args.config == 3 else None,
-        "kernel": "obem_eval_kernel (+ obem_fixup_kernel, < 0.1 % of it) between CUDA events on the launch stream",
+        "kernel": "obem_eval_kernel: one evaluation = its two launches (charges, then panels) + fix-up / repair "
+                  "(< 0.1 %), between CUDA events on the launch stream",
         "peak_source": "derived: %d SMs x %d FP32 lanes x 2 flop x clocks.max.sm %.0f MHz (DESIGN.md); "
                        "MEASURED_PEAKS.json has no FP32 figure" % (sm_count, FP32_LANES_PER_SM, sm_max),
         "flop_per_interaction": FLOP_PER_INTERACTION, "interactions_per_launch": my_inter,
@@ -558,8 +559,9 @@ def bench_next4(torch, api, ctx, wl, timed, dev):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from
-# the `ncu --set full` capture summarised in profiles/r01b_summary.md: 42,320,384 B read + 2,326,016 B written.
-TRAFFIC_BYTES_PER_LAUNCH = 42320384 + 2326016
+# the `ncu --set full` captures summarised in profiles/r01c_summary.md (one launch per source section since r01c):
+# N-body launch 33,781,504 B read + 569,088 B written, panel launch 44,770,048 B read + 187,648 B written.
+TRAFFIC_BYTES_PER_LAUNCH = 33781504 + 569088 + 44770048 + 187648
 
 
 def main():
