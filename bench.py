@@ -157,6 +157,22 @@ def oracle_sample_rate(wl, seconds: float, seed: int = 123):
     return rate, cores, desc, ts
 
 
+def oracle_one_thread_rate(wl, per_core_rate: float, seconds: float = 3.0, seed: int = 321) -> float:
+    """The same oracle on ONE thread (SURVEY.md 8d asks for both), on a sample sized for ~3 s."""
+    from oracle import ref
+    rng = np.random.default_rng(seed)
+    nt = wl.n_targets
+    per_target = (wl.n_charges - (1 if wl.points is None else 0)) + 7 * wl.n_panels
+    n_s = int(min(nt, max(8, seconds * per_core_rate / per_target)))
+    idx = np.sort(rng.choice(nt, n_s, replace=False))
+    tg = (wl.points if wl.points is not None else wl.xyzq)[idx]
+    t0 = time.perf_counter()
+    ref.eval_field(xyzq=wl.xyzq, verts=wl.verts, sigma=wl.sigma, targets=tg,
+                   self_index=idx.astype(np.int64) if wl.points is None else None,
+                   eps_pp=wl.eps_pp, eps_panel=wl.eps_panel, n_threads=1)
+    return n_s * per_target / max(time.perf_counter() - t0, 1e-9)
+
+
 def workload_config(wl, args, world):
     return {
         "workload": "BASELINE.json configs[%d] '%s': %d charges (e-/ions), %d triangular panels, Plummer eps %.3g m; "
@@ -394,7 +410,8 @@ def run_ours(args):
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         rate, cores, desc, _ = oracle_sample_rate(wl, args.cpu_seconds)
-        cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+        cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                        "value_1_thread": oracle_one_thread_rate(wl, rate / cores) / 1e9}
 
     if rank == 0:
         line = {
