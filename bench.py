@@ -240,7 +240,7 @@ def run_ours(args):
 
     wl = W.make_workload(args.config)           # every rank generates the same seeded inputs
     if wl.points is not None:
-        raise SystemExit("bench.py times evaluation at the charges (configs 1-4); config 5 is a parity case")
+        return run_map(args, torch, dist, api, wl, rank, world, local, dev)
     n, npan = wl.n_charges, wl.n_panels
     first, count = shard_range(n, world, rank)
     per_target = (n - 1) + 7 * npan
@@ -431,6 +431,136 @@ def run_ours(args):
             "wall_s_timed_region": wall,
         }
         line.update(extras)
+        print(json.dumps(line), flush=True)
+    ctx.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_map(args, torch, dist, api, wl, rank, world, local, dev):
+    """Config 5, the field map (Table 1): panel -> point sums only, E and phi at every grid point.
+    A step = set_panels + eval_at_points(OBEM_PANELS) over the rank's contiguous slice of the points (weak in
+    nothing: total work fixed, points sharded, panels replicated)."""
+    m, npan = wl.n_targets, wl.n_panels
+    first, count = shard_range(m, world, rank)
+    per_target = 7 * npan
+    total_inter, my_inter = m * per_target, count * per_target
+    ctx = api.Context(local)
+    ctx.reserve(0, npan)
+    ctx.set_softening(wl.eps_pp, wl.eps_panel)
+    d_verts = torch.from_numpy(wl.verts).to(dev)
+    d_sigma = torch.from_numpy(wl.sigma).to(dev)
+    d_pts = torch.from_numpy(wl.points[first:first + count]).to(dev)
+    out = torch.empty((count, 4), dtype=torch.float32, device=dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)  # noqa: E731
+
+    def step(t=None):
+        flush.zero_()
+        if t is not None:
+            t[0].record(stream)
+        ctx.set_panels(d_verts, d_sigma)
+        if t is not None:
+            t[1].record(stream)
+        ctx.eval_at_points(d_pts, out=out, flags=api.PANELS)
+        if t is not None:
+            t[2].record(stream)
+
+    def sync_all():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    sync_all()
+    uuid = getattr(torch.cuda.get_device_properties(local), "uuid", None)
+    sampler = ClockSampler("GPU-%s" % uuid if uuid else str(local))
+    if rank == 0:
+        sampler.start()
+    launches0 = ctx.kernel_launches
+    timers = [[ev(), ev(), ev()] for _ in range(args.steps)]
+    sync_all()
+    wall0 = time.perf_counter()
+    for k in range(args.steps):
+        step(timers[k])
+    sync_all()
+    wall = time.perf_counter() - wall0
+    launches = ctx.kernel_launches - launches0
+    clocks = sampler.stop() if rank == 0 else {}
+    tot_ms = torch.tensor([sum(t[0].elapsed_time(t[2]) for t in timers)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tot_ms, op=dist.ReduceOp.MAX)
+    ms_per_step = float(tot_ms.item()) / max(args.steps, 1)
+    value = total_inter / (ms_per_step * 1e-3) / 1e9
+    eval_s = float(np.mean([t[1].elapsed_time(t[2]) for t in timers])) * 1e-3
+
+    # end to end: ONE C-ABI call with host pointers (H2D of points and panels, set_panels, eval, D2H of the map)
+    h_p = torch.from_numpy(wl.points[first:first + count]).pin_memory()
+    h_v = torch.from_numpy(wl.verts).pin_memory()
+    h_s = torch.from_numpy(wl.sigma).pin_memory()
+    h_out = torch.empty((count, 4), dtype=torch.float32).pin_memory()
+
+    def e2e_step():
+        ctx.field_at_points_host(h_p.numpy(), h_v.numpy(), h_s.numpy(), out=h_out.numpy(), flags=api.PANELS)
+
+    e2e_step()
+    sync_all()
+    t0 = time.perf_counter()
+    e2e_step()
+    sync_all()
+    e2e_s = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_s, op=dist.ReduceOp.MAX)
+
+    sm_max = (clocks.get("sm_max_mhz") or 1965.0) if rank == 0 else 1965.0
+    peak = ctx.sm_count * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+    achieved = FLOP_PER_INTERACTION * my_inter / eval_s / 1e12
+    alg_bytes = 128 * npan + 32 * count
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        rate, cores, desc, _ = oracle_sample_rate(wl, args.cpu_seconds)
+        cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                        "value_1_thread": oracle_one_thread_rate(wl, rate / cores) / 1e9}
+    if rank == 0:
+        cfg = workload_config(wl, args, world)
+        cfg["workload"] = ("BASELINE.json configs[4] '%s': %d grid points, %d triangular panels; E and phi at every "
+                           "point, panel-to-point only" % (wl.name, m, npan))
+        cfg["step"] = "set_panels + eval_at_points(PANELS)"
+        line = {
+            "metric": "G point-source interactions/s (field map: 7 quadrature sources x panels x points)",
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": cfg,
+            "field_evals_per_s": m / (ms_per_step * 1e-3),
+            "pct_fp32_peak": 100.0 * FLOP_PER_INTERACTION * value * 1e9 / 1e12 / (peak * world),
+            "clocks": clocks,
+            "e2e": {"value": total_inter / float(e2e_s.item()) / 1e9, "unit": UNIT,
+                    "h2d_bytes_per_step": (h_p.numel() + h_v.numel() + h_s.numel()) * 4,
+                    "d2h_bytes_per_step": h_out.numel() * 4,
+                    "api": "obem_field_at_points_host (one C-ABI call, pinned host buffers)"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "obem_eval_kernel<panels> (+ fix-up / repair) between CUDA events",
+                         "flop_per_interaction": FLOP_PER_INTERACTION, "interactions_per_launch": my_inter,
+                         "avg_launch_ms": eval_s * 1e3, "algorithmic_bytes_per_launch": alg_bytes,
+                         "achieved_hbm_gbs": alg_bytes / eval_s / 1e9},
+            "cpu_baseline": cpu_baseline, "wall_s_timed_region": wall,
+        }
+        if world == 1 and not args.no_next:
+            a, b = ev(), ev()
+            ctx.eval_at_points(d_pts, out=out, flags=api.PANELS | api.PANELS_EXACT)   # builds the cell lists
+            torch.cuda.synchronize()
+            flush.zero_()
+            a.record(stream)
+            ctx.eval_at_points(d_pts, out=out, flags=api.PANELS | api.PANELS_EXACT)
+            b.record(stream)
+            torch.cuda.synchronize()
+            t_ex = a.elapsed_time(b) * 1e-3
+            line["next3"] = {"panels_exact": {"s": t_ex, "overhead_vs_7_point_only": t_ex / eval_s - 1.0,
+                                              "cell_list_entries": ctx.near_list_size, "cells": ctx.near_cells}}
         print(json.dumps(line), flush=True)
     ctx.destroy()
     if world > 1:
