@@ -706,9 +706,9 @@ def bench_next4(torch, api, ctx, wl, timed, dev):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from
-# the `ncu --set full` captures summarised in profiles/r01c_summary.md (one launch per source section since r01c):
-# N-body launch 33,781,504 B read + 569,088 B written, panel launch 44,770,048 B read + 187,648 B written.
-TRAFFIC_BYTES_PER_LAUNCH = 33781504 + 569088 + 44770048 + 187648
+# the `ncu --set full` captures summarised in profiles/r01d_summary.md (one launch per source section):
+# N-body launch 33.78 MB read + 0.27 MB written, panel launch 44.75 MB read + 0.22 MB written.
+TRAFFIC_BYTES_PER_LAUNCH = 33780000 + 268300 + 44750000 + 215600
 
 
 def main():

@@ -42,7 +42,7 @@ namespace {
 #define OBEM_UNR 4
 #endif
 #ifndef OBEM_DEPTH
-#define OBEM_DEPTH 4
+#define OBEM_DEPTH 3 /* re-swept after the per-section split: 1..8 -> 418.1 415.0 412.7 420.5 413.1 413.1 - 413.1 ms (N-body, config 3) */
 #endif
 constexpr int THREADS = OBEM_THREADS;  /* threads per CTA of the evaluation kernel                 */
 constexpr int TPT = OBEM_TPT;         /* targets per thread                                        */
