@@ -202,3 +202,33 @@ def test_runs_on_a_side_stream(torch_cuda, api, ctx, ref):
     s.synchronize()
     on, op = ref.eval_field(xyzq=xyzq, verts=verts, sigma=sigma, eps_pp=0.05 * UM)
     assert_parity(out.cpu().numpy(), on + op, "side stream")
+
+
+def test_a_time_step_can_be_captured_in_a_cuda_graph(torch_cuda, api, ctx):
+    """Every entry point only enqueues work on the caller's stream (no hidden synchronisation, no allocation once the
+    buffers have their size), so a whole time step -- set_charges + N-body + panels + Euler update -- can be captured
+    in a CUDA graph and replayed; the replay gives bit-identical results."""
+    torch = torch_cuda
+    wl = W.make_workload(1)
+    ctx.set_softening(wl.eps_pp, wl.eps_panel)
+    ctx.set_panels(dev(torch, wl.verts), dev(torch, wl.sigma))
+    x0 = dev(torch, wl.xyzq)
+    v0 = torch.zeros_like(x0)
+    v0[:, 3] = 9.1093837015e-31
+    # eager reference: two Euler steps (also sizes every library-owned buffer)
+    xe, ve = x0.clone(), v0.clone()
+    ctx.step_euler(xe, ve, 25e-15)
+    ctx.step_euler(xe, ve, 25e-15)
+    torch.cuda.synchronize()
+    xg, vg = x0.clone(), v0.clone()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(g, stream=s):
+            ctx.step_euler(xg, vg, 25e-15, stream=s)
+    xg.copy_(x0), vg.copy_(v0)                    # capture does not execute: reset the state, then replay twice
+    g.replay()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(xg, xe) and torch.equal(vg, ve)
