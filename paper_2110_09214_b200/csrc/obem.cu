@@ -48,6 +48,20 @@ constexpr int THREADS = OBEM_THREADS;  /* threads per CTA of the evaluation kern
 constexpr int TPT = OBEM_TPT;         /* targets per thread                                        */
 constexpr int NPAIR = TPT / 2;        /* packed f32x2 target pairs per thread                      */
 constexpr int TT = THREADS * TPT;     /* targets per tile                                          */
+/* The panel launch has its own kernel (obem_panels_kernel) with more targets per thread: measured on config 3,
+ * TPT 10 at pipeline distance 5: 192.9 ms against 196.6 ms at TPT 8; the N-body loop does not gain from it, and its
+ * kernel is left textually alone (its ptxas schedule moves by +-2 % with any change to the shared template). */
+#ifndef OBEM_PANEL_TPT
+#define OBEM_PANEL_TPT 10
+#endif
+#ifndef OBEM_PANEL_DEPTH
+#define OBEM_PANEL_DEPTH 5
+#endif
+constexpr int PANEL_NPAIR = OBEM_PANEL_TPT / 2;
+constexpr int PANEL_DEPTH = OBEM_PANEL_DEPTH;
+constexpr int PANEL_TT = THREADS * OBEM_PANEL_TPT;
+constexpr int TT_MAX = PANEL_TT > TT ? PANEL_TT : TT; /* workspace slots are sized for the larger tile */
+static_assert(OBEM_PANEL_TPT % 2 == 0, "bad tuning knobs");
 constexpr int SB = 256;               /* sources per shared-memory block (4 KiB)                   */
 constexpr int STAGES = 4;             /* depth of the TMA ring                                     */
 constexpr int CTAS_PER_SM = OBEM_CTAS;
@@ -114,6 +128,9 @@ struct EvalParams {
     const long long* U_dev; /* LIST: the unit count lives on the device (no host round trip when the lists are built) */
     unsigned* bad_count;  /* number of targets whose result came out non-finite (see obem_repair_kernel) */
     long long* bad_list;  /* their indices, at most BAD_CAP                                               */
+    /* appended (the point kernel's parameter offsets stay as they were): geometry of THIS launch for the fix-up and
+     * repair kernels -- targets per thread / per tile, and the stride of a workspace slot */
+    int tpt, tt, ws_stride;
 };
 constexpr unsigned BAD_CAP = 1u << 20;
 
@@ -285,11 +302,13 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
  * (source, target pair) instead of 13, like a uniform point block.  Softening: r2' += a^2 eps^2 (B.y = a^2).
  * A source of weight 0 is stored as a = 0, b = 1e17: u'^3 underflows to exactly 0, c_phi = 0.
  */
-template <bool HAS_EPS>
-__device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
-                                           const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
-                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
+template <bool HAS_EPS, int NP>
+__device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NP],
+                                           const u64 (&Y)[NP], const u64 (&Z)[NP], u64 (&aX)[NP],
+                                           u64 (&aY)[NP], u64 (&aZ)[NP], u64 (&aP)[NP])
 {
+    constexpr int NPAIR = NP;          /* shadows the point kernel's pair count */
+    constexpr int DEPTH = PANEL_DEPTH; /* and its pipeline distance */
     constexpr int K = 7 * NPAIR;
 #pragma unroll 1
     for (int pp = 0; pp < PPB; ++pp) {
@@ -615,6 +634,120 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
     }
 }
 
+/*
+ * The panel launch (a4 + a5): the same persistent stream-K structure as obem_eval_kernel<KIND_PANELS>, as a kernel of
+ * its own with NP target pairs per thread (tile = THREADS * 2 NP targets).  No self term, no partner tracking, no
+ * lists: panels only.
+ */
+template <int NP>
+__global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_panels_kernel(const EvalParams P)
+{
+    constexpr int TTP = THREADS * 2 * NP;
+    __shared__ __align__(128) float4 ring[STAGES][SBH_P];
+    __shared__ __align__(8) u64 full[STAGES];
+
+    const int tid = threadIdx.x;
+    const long long G = gridDim.x, c = blockIdx.x;
+    const long long u0 = unit_begin(c, P.U, G), u1 = unit_begin(c + 1, P.U, G);
+    if (u0 >= u1) return;
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&full[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    const unsigned bytes = (unsigned)(SBH_P * sizeof(float4));
+    long long pu = u0, pblk = u0 % P.nblk; /* producer (thread 0): next unit and its block */
+    if (tid == 0) {
+        for (int s = 0; s < STAGES - 1 && pu < u1; ++s) {
+            mbar_expect_tx(&full[s], bytes);
+            tma_load_1d(&ring[s][0], P.sec[0].src + pblk * SBH_P, bytes, &full[s]);
+            ++pu;
+            if (++pblk == P.nblk) pblk = 0;
+        }
+    }
+    const float ke = (float)KE_D;
+    const float eps2 = P.sec[0].eps2;
+    long long u = u0;
+    unsigned it = 0;
+    while (u < u1) {
+        const long long tile = u / P.nblk;
+        const long long b0 = u - tile * P.nblk;
+        const long long nrun = min(P.nblk - b0, u1 - u);
+        const long long tbase = tile * (long long)TTP + tid;
+        const bool whole = (b0 == 0 && nrun == P.nblk);
+        u64 X[NP], Y[NP], Z[NP];
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
+            const float* ta = (const float*)(P.tgt + i0);
+            const float* tb = (const float*)(P.tgt + i1);
+            const bool va = i0 < P.nt, vb = i1 < P.nt;
+            X[p] = pk_keep(va ? __ldg(ta + 0) : 0.f, vb ? __ldg(tb + 0) : 0.f);
+            Y[p] = pk_keep(va ? __ldg(ta + 1) : 0.f, vb ? __ldg(tb + 1) : 0.f);
+            Z[p] = pk_keep(va ? __ldg(ta + 2) : 0.f, vb ? __ldg(tb + 2) : 0.f);
+        }
+        u64 RX[NP], RY[NP], RZ[NP], RP[NP];
+#pragma unroll
+        for (int p = 0; p < NP; ++p) RX[p] = RY[p] = RZ[p] = RP[p] = 0ull;
+
+        for (long long r = 0; r < nrun; ++r, ++it) {
+            __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
+            if (tid == 0 && pu < u1) {
+                const int ps = (it + STAGES - 1) % STAGES;
+                mbar_expect_tx(&full[ps], bytes);
+                tma_load_1d(&ring[ps][0], P.sec[0].src + pblk * SBH_P, bytes, &full[ps]);
+                ++pu;
+                if (++pblk == P.nblk) pblk = 0;
+            }
+            const int st = it % STAGES;
+            mbar_wait(&full[st], (it / STAGES) & 1u);
+            u64 aX[NP], aY[NP], aZ[NP], aP[NP];
+#pragma unroll
+            for (int p = 0; p < NP; ++p) aX[p] = aY[p] = aZ[p] = aP[p] = 0ull;
+            const float4* sblk = &ring[st][1];
+            if (eps2 != 0.f) panel_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            else panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+#pragma unroll
+            for (int p = 0; p < NP; ++p) { /* second accumulation level */
+                RX[p] = add2(RX[p], aX[p]);
+                RY[p] = add2(RY[p], aY[p]);
+                RZ[p] = add2(RZ[p], aZ[p]);
+                RP[p] = add2(RP[p], aP[p]);
+            }
+        }
+
+        float4* wsl = P.ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT_MAX + tid;
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            float4 a, b;
+            upk(RX[p], a.x, b.x);
+            upk(RY[p], a.y, b.y);
+            upk(RZ[p], a.z, b.z);
+            upk(RP[p], a.w, b.w);
+            if (whole) {
+                const long long idx[2] = {tbase + (2 * p) * THREADS, tbase + (2 * p + 1) * THREADS};
+                const float4 v[2] = {a, b};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    if (idx[h] >= P.nt) continue;
+                    float4 o = make_float4(ke * v[h].x, ke * v[h].y, ke * v[h].z, ke * v[h].w);
+                    if (P.accumulate) {
+                        const float4 q = P.out[idx[h]];
+                        o = make_float4(o.x + q.x, o.y + q.y, o.z + q.z, o.w + q.w);
+                    }
+                    P.out[idx[h]] = o;
+                    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, idx[h]);
+                }
+            } else {
+                wsl[(2 * p) * THREADS] = a;
+                wsl[(2 * p + 1) * THREADS] = b;
+            }
+        }
+        u += nrun;
+    }
+}
+
 /* first float4 (the frame origin) of panel p inside the blocked panel buffer */
 __device__ __forceinline__ long long panel_entry(long long p)
 {
@@ -656,16 +789,16 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
     const long long uB = (LIST ? P.tile_ptr[tile + 1] : uA + P.nblk) - 1;
     const int tid = threadIdx.x;
     if (uB < uA) { /* LIST: a tile with no unit at all */
-        for (int k = 0; k < TPT; ++k) {
-            const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
+        for (int k = 0; k < P.tpt; ++k) {
+            const long long i = tile * (long long)P.tt + (long long)k * THREADS + tid;
             if (i < P.nt && !P.accumulate) P.out[i] = make_float4(0.f, 0.f, 0.f, 0.f);
         }
         return;
     }
     const long long cA = cta_of(uA, Utot, G), cB = cta_of(uB, Utot, G);
     if (cA == cB) return; /* one CTA had the whole tile and wrote it directly */
-    for (int k = 0; k < TPT; ++k) {
-        const long long i = tile * (long long)TT + (long long)k * THREADS + tid;
+    for (int k = 0; k < P.tpt; ++k) {
+        const long long i = tile * (long long)P.tt + (long long)k * THREADS + tid;
         if (i >= P.nt) continue;
         double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
         float tm = __int_as_float(0x7f800000);
@@ -675,13 +808,13 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
             if (c0 >= c1) continue;
             const int slot = (c0 >= uA && c0 <= uB) ? 0 : 1; /* the CTA's range STARTS inside this tile */
             if (P.trk_out) { /* CTAs in ascending block order: strict < keeps the lowest block on ties */
-                const float2 t = P.trk_ws[((size_t)c * 2 + slot) * TT + (size_t)k * THREADS + tid];
+                const float2 t = P.trk_ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
                 if (t.x < tm) {
                     tm = t.x;
                     tb = __float_as_int(t.y);
                 }
             }
-            const float4 v = P.ws[((size_t)c * 2 + slot) * TT + (size_t)k * THREADS + tid];
+            const float4 v = P.ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
             ex += (double)v.x;
             ey += (double)v.y;
             ez += (double)v.z;
@@ -772,7 +905,7 @@ __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P
             if (P.list != nullptr) {
                 if (sct != 0) continue;
                 /* LIST mode: the sources of target i are the blocks of its tile's list */
-                const long long tl = i / TT, self = P.self_first >= 0 ? P.self_first + i : -1;
+                const long long tl = i / P.tt, self = P.self_first >= 0 ? P.self_first + i : -1;
                 for (long long j = P.tile_ptr[tl] * SB + tid; j < P.tile_ptr[tl + 1] * SB; j += THREADS) {
                     const long long blk = P.list[j / SB];
                     const float4 q = P.pool[blk * SBH + 1 + (j % SB)];
@@ -1153,6 +1286,9 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     P.nblk = P.sec[0].nblk + P.sec[1].nblk;
     P.tgt = tgt;
     P.nt = nt;
+    P.tpt = TPT;
+    P.tt = TT;
+    P.ws_stride = TT;
     P.ntiles = ceil_div(nt, TT);
     P.U = P.ntiles * P.nblk;
     P.out = out;
@@ -1171,12 +1307,18 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
         Q.sec[1].src = nullptr;
         Q.sec[1].nblk = 0;
         Q.nblk = Q.sec[0].nblk;
+        if (Q.sec[0].kind == KIND_PANELS) { /* the panel launch has its own tile size */
+            Q.tpt = 2 * PANEL_NPAIR;
+            Q.tt = PANEL_TT;
+            Q.ws_stride = TT_MAX;
+            Q.ntiles = ceil_div(nt, (long long)PANEL_TT);
+        }
         Q.U = Q.ntiles * Q.nblk;
         Q.accumulate = (k > 0);
         if (Q.sec[0].kind == KIND_PANELS) {
             Q.self_first = -1;
             Q.trk_out = nullptr;
-            obem_eval_kernel<KIND_PANELS, false><<<c->grid, THREADS, 0, st>>>(Q);
+            obem_panels_kernel<PANEL_NPAIR><<<c->grid, THREADS, 0, st>>>(Q);
         } else if (Q.trk_out) {
             obem_eval_kernel<KIND_POINTS, true><<<c->grid, THREADS, 0, st>>>(Q);
         } else {
@@ -1215,6 +1357,9 @@ int obem_eval_list(obem_ctx* c, const float4* tgt, long long nt, float4* out, co
     P.nblk = 1;
     P.tgt = tgt;
     P.nt = nt;
+    P.tpt = TPT;
+    P.tt = TT;
+    P.ws_stride = TT;
     P.ntiles = ceil_div(nt, TT);
     P.U = 0;
     P.out = out;
@@ -1290,8 +1435,8 @@ int obem_create(obem_ctx** out, int device)
     }
     if (per_sm > CTAS_PER_SM) per_sm = CTAS_PER_SM;
     c->grid = c->sm_count * per_sm;
-    e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT * sizeof(float4));
-    if (e == cudaSuccess) e = cudaMalloc(&c->d_trk_ws, (size_t)c->grid * 2 * TT * sizeof(float2));
+    e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT_MAX * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&c->d_trk_ws, (size_t)c->grid * 2 * TT_MAX * sizeof(float2));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_sink, 256);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_count, 256);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_list, (size_t)BAD_CAP * sizeof(long long));
