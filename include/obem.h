@@ -298,8 +298,9 @@ int obem_interp_map(obem_ctx* c, const float* d_map, int nx, int ny, int nz, con
  * The paper gives no algorithm; reading A19 is: equal-count k-d partition into leaves of 256 charges
  * (stable sorts along the longest box axis, cuts at multiples of 256); per leaf a bounding box and two
  * pseudo-particles (centres of charge of its positive / negative members); for a tile of 2048 consecutive charges
- * (8 leaves) leaf l is FAR iff theta^2 * dist2(box_tile, box_l) > diag2(box_l); near leaves are summed exactly
- * (Eq 3.8, softened, self excluded by index), far leaves through their pseudo-particles (same softening).
+ * (8 leaves) a box B is FAR iff theta^2 * dist2(box_tile, B) > diag2(B); near leaves are summed exactly (Eq 3.8,
+ * softened, self excluded by index), far leaves through their pseudo-particles (same softening); super-leaves (64
+ * leaves) that are far at theta / 2 stand for all their leaves with their own two pseudo-particles.
  * Error ~ theta^2 (the leaves' quadrupoles): measured on config 3 at theta = 2: E rel-L2 2.2e-3 against the exact
  * sum for 3 % of its pair interactions.  theta = 0 is the exact sum.
  * ---------------------------------------------------------------------------------------------------------- */

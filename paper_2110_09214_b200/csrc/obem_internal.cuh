@@ -120,9 +120,13 @@ struct obem_nn_state {
     size_t perm_cap[2] = {0, 0}, key_cap[2] = {0, 0};
     unsigned* seg = nullptr;         /* [2][n_leaf][3] ordered min / max coordinates of the segments of a level */
     float4* sorted = nullptr;        /* [n_leaf * 256] the charges in k-d order (padded): the targets           */
-    float4* pool = nullptr;          /* [(n_leaf + n_group * far_blocks)][OBEM_SBH] leaf blocks, then far blocks */
+    float4* pool = nullptr;          /* [(n_leaf + n_group * far_cap)][OBEM_SBH] leaf blocks, then far blocks */
     float* leafbox = nullptr;        /* [n_leaf][6] */
     float4* pseudo = nullptr;        /* [n_leaf][2] centre of charge of the positive / negative members         */
+    double* leafmom = nullptr;       /* [n_leaf][8] Q+, Q+ R+, Q-, Q- R- in fp64 (for the super-leaves)          */
+    float* superbox = nullptr;       /* [n_super][6] */
+    float4* superpseudo = nullptr;   /* [n_super][2] */
+    size_t leafmom_cap = 0, superbox_cap = 0, superpseudo_cap = 0;
     long long* cnt = nullptr;        /* [n_group] units of each tile */
     long long* tile_ptr = nullptr;   /* [n_group + 1] + the unit count U */
     int* list = nullptr;

@@ -8,13 +8,14 @@
  *      (stably) along the longest axis of its bounding box and cut at a multiple of 256 -- one radix sort per level
  *      over the whole array with key = (segment start, coordinate).  A leaf = 256 charges = one source block of the
  *      evaluation kernel; a target group = 8 consecutive leaves = one 2048-target tile.
- *   2. Per leaf: bounding box and two pseudo-particles (the centres of charge of its positive and of its negative
- *      members).
- *   3. Per (tile, leaf): FAR iff theta^2 dist2(box_tile, box_leaf) > diag2(box_leaf), decided in fp64 with
- *      individually rounded operations (the oracle takes the same decisions bit for bit).
+ *   2. Per leaf, and per super-leaf (64 consecutive leaves): bounding box and two pseudo-particles (the centres of
+ *      charge of its positive and of its negative members).
+ *   3. A box B is FAR from tile t iff theta^2 dist2(box_t, B) > diag2(B), decided in fp64 with individually rounded
+ *      operations (the oracle takes the same decisions bit for bit).  A super-leaf that is far at theta / 2 stands for
+ *      all its leaves; the leaves of the other super-leaves are classified one by one at theta.
  *   4. Tile t's source list = its near leaves (the charges themselves, exact Eq 3.8, self excluded by index) + its
- *      own copy of all pseudo-particles with the near leaves' ones blanked -- run by the LIST instantiation of the
- *      hot path's evaluation kernel (obem.cu), stream-K over all (tile, block) units.
+ *      own far blocks: the pseudo-particles of its far super-leaves and far leaves, compacted -- run by the LIST
+ *      instantiation of the hot path's evaluation kernel (obem.cu), stream-K over all (tile, block) units.
  *   5. Results are scattered back to the input order.
  *
  * Every step is enqueued on the caller's stream; nothing is read back to the host (all sizes follow from n).
@@ -30,7 +31,8 @@ typedef unsigned long long u64k;
 constexpr int LEAF = OBEM_SB;        /* 256 */
 constexpr int GROUP = OBEM_TT;       /* 2048 */
 constexpr int LPG = GROUP / LEAF;    /* leaves per group */
-constexpr int PPB_FAR = LEAF / 2;    /* leaves whose two pseudo-particles fill one far block */
+constexpr int SUPER = 64;            /* leaves per super-leaf */
+constexpr int MAX_SUPER = 32768;     /* super-leaves the list kernel keeps flags for (5.4e8 charges) */
 constexpr float NN_PAD_FAR = 1.0e15f;
 
 __host__ __device__ __forceinline__ long long nn_split(long long a, long long b)
@@ -165,7 +167,7 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
 __global__ void __launch_bounds__(LEAF) nn_leaf_kernel(const float4* __restrict__ x, const int* __restrict__ perm,
                                                         long long n, float4* __restrict__ sorted,
                                                         float4* __restrict__ pool, float* __restrict__ leafbox,
-                                                        float4* __restrict__ pseudo)
+                                                        float4* __restrict__ pseudo, double* __restrict__ leafmom)
 {
     __shared__ double red[8][LEAF / 32];
     __shared__ float fred[6][LEAF / 32];
@@ -212,6 +214,7 @@ __global__ void __launch_bounds__(LEAF) nn_leaf_kernel(const float4* __restrict_
             for (int k = 0; k < 8; ++k) red[k][0] += red[k][ww];
         }
         for (int d = 0; d < 6; ++d) leafbox[l * 6 + d] = fred[d][0];
+        for (int k = 0; k < 8; ++k) leafmom[l * 8 + k] = red[k][0]; /* Q+, Q+ R+ (3), Q-, Q- R- (3): for the super-leaves */
         for (int h = 0; h < 2; ++h) {
             const double Q = red[4 * h][0];
             pseudo[l * 2 + h] = (Q != 0.0) ? make_float4((float)(red[4 * h + 1][0] / Q), (float)(red[4 * h + 2][0] / Q),
@@ -249,56 +252,119 @@ __device__ __forceinline__ void nn_group_box(const float* __restrict__ leafbox, 
         }
 }
 
-/* one CTA per group.  FILL = false: cnt[g] = (near leaves) + (far blocks).  FILL = true: write the group's list
- * (near leaf blocks in ascending order, then its far blocks) and its far blocks (all pseudo-particles, the near
- * leaves' ones blanked). */
+/* one thread per super-leaf: union of its leaves' boxes, centres of charge from their fp64 moments (leaf order) */
+__global__ void nn_super_kernel(const float* __restrict__ leafbox, const double* __restrict__ leafmom, long long n_leaf,
+                                long long n_super, float* __restrict__ superbox, float4* __restrict__ superpseudo)
+{
+    const long long sidx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (sidx >= n_super) return;
+    const float big = __int_as_float(0x7f800000);
+    float b[6] = {big, big, big, -big, -big, -big};
+    double m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (long long l = sidx * SUPER; l < (sidx + 1) * SUPER && l < n_leaf; ++l) {
+        for (int d = 0; d < 3; ++d) {
+            b[d] = fminf(b[d], leafbox[l * 6 + d]);
+            b[3 + d] = fmaxf(b[3 + d], leafbox[l * 6 + 3 + d]);
+        }
+        for (int k = 0; k < 8; ++k) m[k] += leafmom[l * 8 + k];
+    }
+    for (int d = 0; d < 6; ++d) superbox[sidx * 6 + d] = b[d];
+    for (int h = 0; h < 2; ++h) {
+        const double Q = m[4 * h];
+        superpseudo[sidx * 2 + h] = (Q != 0.0) ? make_float4((float)(m[4 * h + 1] / Q), (float)(m[4 * h + 2] / Q),
+                                                             (float)(m[4 * h + 3] / Q), (float)Q)
+                                               : make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
+    }
+}
+
+/* entry e of a tile's far area (blocks of 256 entries, each behind a header) */
+__device__ __forceinline__ float4* nn_far_slot(float4* far, long long e) { return far + (e >> 8) * OBEM_SBH + 1 + (e & 255); }
+
+/* block-wide rank of the threads whose flag is set (ascending thread order) and their total; wsum: 8 ints of scratch */
+__device__ __forceinline__ int nn_block_rank(bool flag, int* wsum, int& total)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const unsigned bal = __ballot_sync(0xffffffffu, flag);
+    __syncthreads(); /* wsum is free again */
+    if (lane == 0) wsum[w] = __popc(bal);
+    __syncthreads();
+    int before = 0;
+    total = 0;
+    for (int ww = 0; ww < 8; ++ww) {
+        if (ww < w) before += wsum[ww];
+        total += wsum[ww];
+    }
+    return before + __popc(bal & ((1u << lane) - 1u));
+}
+
+/* one CTA per tile.  FILL = false: cnt[g] = (near leaves) + (far blocks).  FILL = true: write the tile's list (near
+ * leaf blocks in ascending order, then its far blocks) and its far blocks: the pseudo-particles of its far
+ * super-leaves (ascending), then of its far leaves (ascending), padded with blanks to a whole block. */
 template <bool FILL>
 __global__ void __launch_bounds__(256) nn_lists_kernel(const float* __restrict__ leafbox, const float4* __restrict__ pseudo,
-                                                       long long n_leaf, long long far_blocks, double theta2,
+                                                       const float* __restrict__ superbox,
+                                                       const float4* __restrict__ superpseudo, long long n_leaf,
+                                                       long long n_super, long long far_cap, double theta2,
+                                                       double theta2_super,
                                                        long long* __restrict__ cnt, const long long* __restrict__ tile_ptr,
                                                        int* __restrict__ list, float4* __restrict__ pool)
 {
     __shared__ int wsum[8];
-    __shared__ int base_sh;
+    __shared__ unsigned sflag[MAX_SUPER / 32]; /* bit s: super-leaf s is far from this tile */
     const long long g = blockIdx.x;
     float gb[6];
     nn_group_box(leafbox, g, n_leaf, gb);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (threadIdx.x == 0) base_sh = 0;
-    __syncthreads();
-    float4* far = FILL ? pool + (n_leaf + g * far_blocks) * OBEM_SBH : nullptr;
+    const int lane = threadIdx.x & 31;
+    float4* far = FILL ? pool + (n_leaf + g * far_cap) * OBEM_SBH : nullptr;
     int* out = FILL ? list + tile_ptr[g] : nullptr;
-    const long long l_end = far_blocks * PPB_FAR; /* leaves incl. the padding of the last far block */
-    for (long long l0 = 0; l0 < l_end; l0 += 256) {
-        const long long l = l0 + threadIdx.x;
-        const bool real = l < n_leaf;
-        const bool near = real && !nn_is_far(gb, leafbox + l * 6, theta2);
-        const unsigned bal = __ballot_sync(0xffffffffu, near);
-        if (lane == 0) wsum[w] = __popc(bal);
-        __syncthreads();
-        int before = base_sh, total = 0;
-        for (int ww = 0; ww < 8; ++ww) {
-            if (ww < w) before += wsum[ww];
-            total += wsum[ww];
+    long long n_far = 0; /* pairs of pseudo-particles in the far area so far (same value in every thread) */
+    int n_near = 0;
+    /* super-leaves */
+    for (long long s0 = 0; s0 < n_super; s0 += 256) {
+        const long long sidx = s0 + threadIdx.x;
+        const bool isfar = sidx < n_super && nn_is_far(gb, superbox + sidx * 6, theta2_super);
+        const unsigned bal = __ballot_sync(0xffffffffu, isfar);
+        if (lane == 0 && (s0 + (threadIdx.x & ~31)) < n_super) sflag[(s0 + threadIdx.x) >> 5] = bal;
+        int total;
+        const int rank = nn_block_rank(isfar, wsum, total);
+        if (FILL && isfar) {
+            *nn_far_slot(far, 2 * (n_far + rank)) = superpseudo[sidx * 2];
+            *nn_far_slot(far, 2 * (n_far + rank) + 1) = superpseudo[sidx * 2 + 1];
         }
+        n_far += total;
+    }
+    __syncthreads();
+    /* leaves of the super-leaves that are not far */
+    for (long long l0 = 0; l0 < n_leaf; l0 += 256) {
+        const long long l = l0 + threadIdx.x;
+        bool near = false, farleaf = false;
+        if (l < n_leaf && !((sflag[(l / SUPER) >> 5] >> ((l / SUPER) & 31)) & 1u)) {
+            farleaf = nn_is_far(gb, leafbox + l * 6, theta2);
+            near = !farleaf;
+        }
+        int tn, tf;
+        const int rn = nn_block_rank(near, wsum, tn);
+        const int rf = nn_block_rank(farleaf, wsum, tf);
         if (FILL) {
-            if (near) out[before + __popc(bal & ((1u << lane) - 1u))] = (int)l;
-            if (l < l_end) {
-                const float4 blank = make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
-                float4* dst = far + (l / PPB_FAR) * OBEM_SBH + 1 + 2 * (l % PPB_FAR);
-                dst[0] = (real && !near) ? pseudo[l * 2] : blank;
-                dst[1] = (real && !near) ? pseudo[l * 2 + 1] : blank;
-                if (l % PPB_FAR == 0) dst[-1] = make_float4(__int_as_float(0x7fc00000), 0.f, 0.f, 0.f); /* header */
+            if (near) out[n_near + rn] = (int)l;
+            if (farleaf) {
+                *nn_far_slot(far, 2 * (n_far + rf)) = pseudo[l * 2];
+                *nn_far_slot(far, 2 * (n_far + rf) + 1) = pseudo[l * 2 + 1];
             }
         }
-        __syncthreads();
-        if (threadIdx.x == 0) base_sh += total;
-        __syncthreads();
+        n_near += tn;
+        n_far += tf;
     }
+    const long long entries = 2 * n_far, blocks = (entries + 255) >> 8;
     if (FILL) {
-        for (long long k = threadIdx.x; k < far_blocks; k += 256) out[base_sh + k] = (int)(n_leaf + g * far_blocks + k);
+        const float4 blank = make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
+        for (long long e = entries + threadIdx.x; e < blocks * 256; e += 256) *nn_far_slot(far, e) = blank;
+        for (long long k = threadIdx.x; k < blocks; k += 256) {
+            far[k * OBEM_SBH] = make_float4(__int_as_float(0x7fc00000), 0.f, 0.f, 0.f); /* header: weights differ */
+            out[n_near + k] = (int)(n_leaf + g * far_cap + k);
+        }
     } else if (threadIdx.x == 0) {
-        cnt[g] = base_sh + far_blocks;
+        cnt[g] = n_near + blocks;
     }
 }
 
@@ -352,7 +418,7 @@ int nn_grow(obem_ctx* c, T*& p, size_t& cap, size_t count)
 void obem_nn_free(obem_ctx* c)
 {
     void* ptrs[] = {c->nn.perm[0], c->nn.perm[1], c->nn.key[0], c->nn.key[1], c->nn.seg, c->nn.sorted, c->nn.pool,
-                    c->nn.leafbox, c->nn.pseudo, c->nn.cnt, c->nn.tile_ptr, c->nn.list, c->nn.out_sorted, c->nn.tmp,
+                    c->nn.leafbox, c->nn.pseudo, c->nn.leafmom, c->nn.superbox, c->nn.superpseudo, c->nn.cnt, c->nn.tile_ptr, c->nn.list, c->nn.out_sorted, c->nn.tmp,
                     c->nn.pan};
     for (void* p : ptrs)
         if (p) cudaFree(p);
@@ -384,7 +450,9 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     cudaStream_t st = (cudaStream_t)cuda_stream;
     obem_nn_state& S = c->nn;
     const long long n_leaf = ceil_div(n, LEAF), n_group = ceil_div(n, GROUP);
-    const long long far_blocks = ceil_div(n_leaf, PPB_FAR);
+    const long long n_super = ceil_div(n_leaf, SUPER);
+    if (n_super > MAX_SUPER) return OBEM_EINVAL;
+    const long long far_cap = ceil_div(2 * (n_leaf + n_super), LEAF); /* far blocks a tile can need at most */
     int levels = 0;
     while ((1LL << levels) < n_leaf) ++levels;
     int nbits = 1;
@@ -397,12 +465,15 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     }
     if (rc == OBEM_OK) rc = nn_grow(c, S.seg, S.seg_cap, (size_t)n_leaf * 6);
     if (rc == OBEM_OK) rc = nn_grow(c, S.sorted, S.sorted_cap, (size_t)n_leaf * LEAF);
-    if (rc == OBEM_OK) rc = nn_grow(c, S.pool, S.pool_cap, (size_t)(n_leaf + n_group * far_blocks) * OBEM_SBH);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.pool, S.pool_cap, (size_t)(n_leaf + n_group * far_cap) * OBEM_SBH);
     if (rc == OBEM_OK) rc = nn_grow(c, S.leafbox, S.leafbox_cap, (size_t)n_leaf * 6);
     if (rc == OBEM_OK) rc = nn_grow(c, S.pseudo, S.pseudo_cap, (size_t)n_leaf * 2);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.leafmom, S.leafmom_cap, (size_t)n_leaf * 8);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.superbox, S.superbox_cap, (size_t)n_super * 6);
+    if (rc == OBEM_OK) rc = nn_grow(c, S.superpseudo, S.superpseudo_cap, (size_t)n_super * 2);
     if (rc == OBEM_OK) rc = nn_grow(c, S.cnt, S.cnt_cap, (size_t)n_group);
     if (rc == OBEM_OK) rc = nn_grow(c, S.tile_ptr, S.tile_ptr_cap, (size_t)n_group + 2); /* [n_group + 1] + U */
-    if (rc == OBEM_OK) rc = nn_grow(c, S.list, S.list_cap, (size_t)n_group * (size_t)(n_leaf + far_blocks));
+    if (rc == OBEM_OK) rc = nn_grow(c, S.list, S.list_cap, (size_t)n_group * (size_t)(n_leaf + far_cap));
     if (rc == OBEM_OK) rc = nn_grow(c, S.out_sorted, S.out_sorted_cap, (size_t)n);
     if (rc != OBEM_OK) return rc;
     size_t tmp_bytes = 0;
@@ -436,20 +507,25 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     }
     const int* perm = S.perm[cur];
     /* 2. leaves */
-    nn_leaf_kernel<<<(unsigned)n_leaf, LEAF, 0, st>>>(c->d_chg, perm, n, S.sorted, S.pool, S.leafbox, S.pseudo);
+    nn_leaf_kernel<<<(unsigned)n_leaf, LEAF, 0, st>>>(c->d_chg, perm, n, S.sorted, S.pool, S.leafbox, S.pseudo,
+                                                      S.leafmom);
+    OBEM_CUDA(c, cudaGetLastError());
+    nn_super_kernel<<<(unsigned)ceil_div(n_super, 64), 64, 0, st>>>(S.leafbox, S.leafmom, n_leaf, n_super, S.superbox,
+                                                                    S.superpseudo);
     OBEM_CUDA(c, cudaGetLastError());
     /* 3. + 4. per-tile lists and far blocks */
     const double theta2 = (double)S.theta * (double)S.theta;
+    const double theta_s = 0.5 * (double)S.theta, theta2s = theta_s * theta_s; /* super-leaves: accepted at theta / 2 */
     long long* U_dev = S.tile_ptr + n_group + 1;
-    nn_lists_kernel<false><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, n_leaf, far_blocks, theta2, S.cnt,
-                                                              nullptr, nullptr, nullptr);
+    nn_lists_kernel<false><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, S.superbox, S.superpseudo, n_leaf,
+                                                              n_super, far_cap, theta2, theta2s, S.cnt, nullptr, nullptr, nullptr);
     OBEM_CUDA(c, cudaGetLastError());
     nn_scan_kernel<<<1, 32, 0, st>>>(S.cnt, n_group, S.tile_ptr, U_dev);
     OBEM_CUDA(c, cudaGetLastError());
-    nn_lists_kernel<true><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, n_leaf, far_blocks, theta2, S.cnt,
-                                                             S.tile_ptr, S.list, S.pool);
+    nn_lists_kernel<true><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, S.superbox, S.superpseudo, n_leaf,
+                                                             n_super, far_cap, theta2, theta2s, S.cnt, S.tile_ptr, S.list, S.pool);
     OBEM_CUDA(c, cudaGetLastError());
-    c->launches += 5;
+    c->launches += 6;
     /* 5. the sums, in sorted order, then back to the input order */
     rc = obem_eval_list(c, S.sorted, n, S.out_sorted, S.pool, S.tile_ptr, S.list, U_dev, n_leaf, c->eps_pp, st);
     if (rc != OBEM_OK) return rc;

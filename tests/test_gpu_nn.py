@@ -67,9 +67,7 @@ def _gpu_nn(torch, ctx, x, eps, theta, flags=1):
 
 
 def _oracle_units(nn, tree, theta, n):
-    n_leaf = tree["leaf_boxes"].shape[0]
-    far_blocks = -(-n_leaf // 128)
-    return sum(int((~nn.far_mask(tree, g, theta)).sum()) + far_blocks for g in range(tree["group_boxes"].shape[0]))
+    return nn.units(tree, theta, n)
 
 
 @pytest.mark.parametrize("n,theta", [(50000, 0.0), (50000, 2.0), (50000, 6.0), (20011, 3.0)])
@@ -88,6 +86,9 @@ def test_matches_the_nn_oracle(torch_cuda, ctx, nn, ref, n, theta):
         n_leaf = tree["leaf_boxes"].shape[0]
         assert any(nn.far_mask(tree, g, theta).any() for g in range(tree["group_boxes"].shape[0])), "no far leaf: vacuous"
         assert n_leaf > 8
+        if n >= 50000 and theta >= 6.0:   # both far levels are exercised
+            cls = [nn.classify(tree, g, theta) for g in range(tree["group_boxes"].shape[0])]
+            assert any(c[0].any() for c in cls) and any(c[2].any() for c in cls)
 
 
 def test_config3_full_size_sampled_groups(torch_cuda, api, ctx, nn, ref):

@@ -144,3 +144,53 @@ def test_n7_paper_fig6_acceptance_on_separated_clouds(nn, ref):
     got, _ = nn.nn_field(x, 0.05 * UM, 2.0, leaf=64, group=512, ref=ref)
     rel = np.abs((got[:, 2] - bf[:, 2]) / bf[:, 2])
     assert (rel < 0.05).mean() > 0.968, (rel < 0.05).mean()
+
+
+def test_n8_two_level_far_hand_value_and_limits(nn, ref):
+    """leaf = group = 2, super-leaf = 2 leaves.  Pair A at the origin; four equal charges B 5 mm away (two leaves,
+    ONE super-leaf whose box is far from A's box): A sees them as ONE pseudo-particle 4q at their centroid.  With
+    super-leaves that are never far (super_ larger than the tree) the result is the one-level one."""
+    u = 100 * UM
+    pts = [[0, 0, 0], [0, 0, 0.3 * u],                                        # A
+           [50 * u, 0.1 * u, 0], [50 * u, -0.1 * u, 0], [50.2 * u, 0.1 * u, 0], [50.2 * u, -0.1 * u, 0],   # B
+           [0, 3 * u, 0], [0.2 * u, 3 * u, 0]]                                 # C: pads A's super-leaf to 2 leaves
+    x = np.zeros((8, 4), dtype=np.float32)
+    x[:, :3] = pts
+    x[:, 3] = [QE, -QE, QE, QE, QE, QE, -QE, QE]
+    q32 = float(x[0, 3])
+    got, tree = nn.nn_field(x, 0.0, 1.0, leaf=2, group=2, super_=2, ref=ref)
+    perm = tree["perm"]
+    # which super-leaf holds B?  the one whose members are input indices 2..5
+    supers = [sorted(perm[4 * k:4 * k + 4].tolist()) for k in range(2)]
+    assert [2, 3, 4, 5] in supers
+    gA = [g for g in range(4) if sorted(perm[2 * g:2 * g + 2].tolist()) == [0, 1]][0]
+    far_super, near, far_leaf = nn.classify(tree, gA, 1.0)
+    assert far_super[supers.index([2, 3, 4, 5])] and not far_super[1 - supers.index([2, 3, 4, 5])]
+    p = x[:, :3].astype(np.float64)
+    cB = p[2:6].mean(axis=0)
+    # A0 = exact partner A1 + 4q at B's centroid + leaf C (far leaf or near: take what classify says)
+    d1, dB = p[0] - p[1], p[0] - cB
+    e = KE * (-q32) * d1 / np.linalg.norm(d1) ** 3 + KE * 4 * q32 * dB / np.linalg.norm(dB) ** 3
+    lC = [l for l in range(4) if sorted(perm[2 * l:2 * l + 2].tolist()) == [6, 7]][0]
+    for j, qj in ((6, -q32), (7, q32)):                                       # C is (-e, +e): its two pseudo-particles ARE its charges
+        dj = p[0] - p[j]
+        e = e + KE * qj * dj / np.linalg.norm(dj) ** 3
+    assert near[lC] or far_leaf[lC]
+    assert np.allclose(got[0, :3], e, rtol=1e-12)
+    # never-far super-leaves reproduce the one-level scheme
+    rng = np.random.default_rng([51, 8])
+    y = _cloud(rng, 4096)
+    one, t1 = nn.nn_field(y, 0.05 * UM, 4.0, leaf=16, group=128, super_=10 ** 6, ref=ref)
+    two, t2 = nn.nn_field(y, 0.05 * UM, 4.0, leaf=16, group=128, super_=8, ref=ref)
+    assert not any(nn.classify(t1, g, 4.0)[0].any() for g in range(32))
+    assert any(nn.classify(t2, g, 4.0)[0].any() for g in range(32)), "no far super-leaf: vacuous"
+    bf, _ = ref.eval_field(xyzq=y, eps_pp=0.05 * UM, flags=ref.NBODY)
+    err = lambda a: np.sqrt(((a[:, :3] - bf[:, :3]) ** 2).sum() / (bf[:, :3] ** 2).sum())
+    assert err(one) < 5e-2 and err(two) < 5e-2 and err(two) < 2 * err(one)      # super-leaves are accepted at theta / 2
+    assert nn.units(t2, 4.0, 4096, block=16) < nn.units(t1, 4.0, 4096, block=16)
+    # super-leaf pseudo-particles conserve charge and dipole moment as well
+    q = y[:, 3].astype(np.float64)
+    sp = t2["super_pseudo"].reshape(-1, 4)
+    assert abs(sp[:, 3].sum() - q.sum()) <= 1e-12 * np.abs(q).sum()
+    assert np.allclose((sp[:, 3:4] * sp[:, :3]).sum(0), (q[:, None] * y[:, :3].astype(np.float64)).sum(0), rtol=0,
+                       atol=1e-12 * np.abs(q).sum() * 50 * UM)
