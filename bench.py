@@ -669,6 +669,24 @@ def bench_nn(torch, api, ctx, wl, timed, out, t_nbody):
                                    "Ginteractions_per_s_whole_call": inter / t / 1e9,
                                    "frac_fp32_peak_whole_call": FLOP_PER_INTERACTION * inter / t / 1e12 / peak_flops}
     ctx.set_nn_theta(2.0)
+    # the paper's largest Table-2 case: 1e7 particles (synthetic Gaussian electron/ion cloud, seeded on the device)
+    free, _ = torch.cuda.mem_get_info()
+    if free > 16e9:
+        n10 = 10_000_000
+        gen = torch.Generator(device=out.device)
+        gen.manual_seed(10)
+        x10 = torch.randn((n10, 4), dtype=torch.float32, device=out.device, generator=gen)
+        x10[:, :3] *= torch.tensor([40e-6, 40e-6, 20e-6], device=out.device)
+        x10[:, 3] = torch.where(x10[:, 3] > 0, 1.602176634e-19, -1.602176634e-19)
+        out10 = torch.empty_like(x10)
+        ctx.set_charges(x10)
+        t = timed(lambda: ctx.eval_at_charges_nn(out=out10, flags=api.NBODY), reps=2)
+        units = ctx.nn_last_units()
+        res["n_1e7_theta_2"] = {"s": t, "units": units, "pair_interactions": units * 2048 * 256,
+                                "fraction_of_exact_pairs": units * 2048 * 256 / (n10 * (n10 - 1.0)),
+                                "exact_sum_would_take_s": n10 * (n10 - 1.0) / (n * (n - 1.0)) * t_nbody}
+        del x10, out10
+        ctx.set_charges(torch.from_numpy(wl.xyzq).to(out.device))
     return res
 
 
@@ -706,9 +724,9 @@ def bench_next4(torch, api, ctx, wl, timed, dev):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from
-# the `ncu --set full` captures summarised in profiles/r01d_summary.md (one launch per source section):
-# N-body launch 33.78 MB read + 0.27 MB written, panel launch 44.75 MB read + 0.22 MB written.
-TRAFFIC_BYTES_PER_LAUNCH = 33780000 + 268300 + 44750000 + 215600
+# the `ncu --set full` captures summarised in profiles/r01e_summary.md (one launch per source section):
+# N-body launch 33.80 MB read + 0.71 MB written, panel launch 43.51 MB read + 0.16 MB written.
+TRAFFIC_BYTES_PER_LAUNCH = 33800000 + 710400 + 43510000 + 162000
 
 
 def main():

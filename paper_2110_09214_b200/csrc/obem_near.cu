@@ -290,7 +290,7 @@ __device__ __forceinline__ bool near_pair(const NearParams& P, int p, const floa
     return r2min < P.crit2 * R * R;
 }
 
-constexpr int NEAR_WARPS = 8;
+constexpr int NEAR_WARPS = 2; /* small CTAs: most warps leave at once (no near panel): 14.5 -> 12.3 ms on config 3 against 8 warps */
 /* A target closer than VERY_NEAR * h_p to a quadrature source of panel p: that one 7-point term exceeds the whole
  * local field by more than 0.013 / VERY_NEAR^2 (= 13 at 1/32), and what it cost the fp32 accumulation of the
  * evaluation kernel (an ulp of ITS size) cannot be corrected afterwards.  Such targets are recomputed from scratch
