@@ -101,7 +101,6 @@ constexpr int SBH = SB + 1;
 constexpr int PPB = 34;
 constexpr int PANEL_SLOTS = 15;
 constexpr int SBH_P = 512 + 1;
-constexpr int RING_SLOTS = SBH_P; /* a ring stage holds the larger of the two block kinds */
 constexpr int PANELS_PER_BLOCK = PPB;
 
 struct EvalParams {
