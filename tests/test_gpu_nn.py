@@ -115,6 +115,29 @@ def test_config3_full_size_sampled_groups(torch_cuda, api, ctx, nn, ref):
     assert units * 2048 * 256 < 0.06 * wl.n_charges * (wl.n_charges - 1)
 
 
+def test_config4_charges_full_size_sampled_groups(torch_cuda, api, ctx, nn, ref):
+    """4,194,304 charges in two clouds 2 mm apart (config 4): 256 super-leaves, many of them far.  Two sampled tiles
+    against the oracle, identical decisions over all 2048 tiles, and the paper's acceptance against the exact sum."""
+    wl = W.make_workload(4, mesh_div=64)
+    got = _gpu_nn(torch_cuda, ctx, wl.xyzq, wl.eps_pp, 2.0)
+    assert np.isfinite(got).all()
+    units = ctx.nn_last_units()
+    rng = np.random.default_rng([61, 4])
+    groups = np.sort(rng.choice(wl.n_charges // 2048, 2, replace=False))
+    exp, tree = nn.nn_field(wl.xyzq, wl.eps_pp, 2.0, groups=groups, ref=ref)
+    idx = np.nonzero(np.isfinite(exp[:, 0]))[0]
+    assert idx.size == 2 * 2048
+    assert_parity(got[idx], exp[idx], "cfg4 nn, sampled tiles")
+    assert units == _oracle_units(nn, tree, 2.0, wl.n_charges)
+    assert all(nn.classify(tree, g, 2.0)[0].any() for g in groups), "no far super-leaf: vacuous"
+    bf, _ = ref.eval_field(xyzq=wl.xyzq, targets=wl.xyzq[idx], self_index=idx.astype(np.int64), eps_pp=wl.eps_pp,
+                           flags=ref.NBODY)
+    rel = np.abs((got[idx, 2] - bf[:, 2]) / bf[:, 2])
+    assert (rel < 0.05).mean() > 0.968
+    assert field_errors(got[idx], bf)["E_rel_l2"] < 5e-3
+    assert units * 2048 * 256 < 0.02 * wl.n_charges * (wl.n_charges - 1.0)
+
+
 @pytest.mark.parametrize("n", [1, 2, 255, 256, 257, 2047, 2049, 4097])
 def test_small_and_ragged_sizes(torch_cuda, ctx, nn, ref, n):
     rng = np.random.default_rng([61, 7, n])
