@@ -299,7 +299,9 @@ constexpr double VERY_NEAR = 1.0 / 32.0;
 
 /* one warp per target: the lanes test 32 candidates of the target's cell at a time; the near ones are compacted
  * into a per-warp queue so that the expensive closed form always runs on full warps */
-__global__ void __launch_bounds__(NEAR_WARPS * 32) near_correct_kernel(const NearParams P)
+/* latency-bound (dependent fp64 log / atan chains, per-pair loads): more resident warps beat fewer spills -- A/B on config 3
+ * with the register cap of 2..32 CTAs/SM: 12.4 (108 registers), 11.0 (96), 10.1 (72), 8.8 (48), 8.1 (40), 8.6 (32) ms */
+__global__ void __launch_bounds__(NEAR_WARPS * 32, 24) near_correct_kernel(const NearParams P)
 {
     __shared__ int queue[NEAR_WARPS][64];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
