@@ -76,7 +76,8 @@ int obem_reserve(obem_ctx* c, int64_t n_charges, int64_t n_panels);
  * next evaluate call. */
 int obem_set_softening(obem_ctx* c, float eps_pp_m, float eps_panel_m);
 
-/* Panels (flat cells with constant sigma; triangles only, reading A8).
+/* Panels (flat cells with constant sigma; triangles here, quadrilaterals through
+ * obem_set_panels_cells, reading A8).
  *   d_verts [n_panels][3][3] fp32: vertex j of panel p at d_verts[(p*3+j)*3 + 0..2] = x,y,z [m]
  *   d_sigma [n_panels] fp32 [C/m^2]
  * Derives, in fp64 and rounded once to fp32, the area A_p and the 7 quadrature sources
