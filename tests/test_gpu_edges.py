@@ -232,3 +232,27 @@ def test_a_time_step_can_be_captured_in_a_cuda_graph(torch_cuda, api, ctx):
     g.replay()
     torch.cuda.synchronize()
     assert torch.equal(xg, xe) and torch.equal(vg, ve)
+
+
+def test_results_are_bitwise_reproducible_and_independent_of_other_work(torch_cuda, api, ctx):
+    """No atomics on the data path: split tiles are summed in a fixed order by the fix-up kernel, so two evaluations
+    of the same inputs agree bit for bit -- also when other evaluations (other sizes, other contexts) ran in between."""
+    torch = torch_cuda
+    wl = W.make_workload(2, charge_div=2, mesh_div=2)          # 32768 charges: 16 tiles split among 148 CTAs
+    ctx.set_softening(wl.eps_pp, wl.eps_panel)
+    ctx.set_panels(dev(torch, wl.verts), dev(torch, wl.sigma))
+    ctx.set_charges(dev(torch, wl.xyzq))
+    a = ctx.eval_at_charges(flags=api.NBODY | api.PANELS).clone()
+    other = api.Context(0)
+    small = W.make_workload(1)
+    other.set_softening(small.eps_pp, 0.0)
+    other.set_charges(dev(torch, small.xyzq))
+    other.eval_at_charges(flags=api.NBODY)
+    ctx.eval_at_points(dev(torch, wl.xyzq[:1000]), flags=api.PANELS)
+    b = ctx.eval_at_charges(flags=api.NBODY | api.PANELS)
+    ex1 = ctx.eval_at_charges(flags=api.NBODY | api.PANELS | api.PANELS_EXACT).clone()
+    ex2 = ctx.eval_at_charges(flags=api.NBODY | api.PANELS | api.PANELS_EXACT)
+    torch.cuda.synchronize()
+    other.destroy()
+    assert torch.equal(a, b)
+    assert torch.equal(ex1, ex2)
