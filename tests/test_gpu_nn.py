@@ -198,3 +198,23 @@ def test_argument_errors(torch_cuda, api, ctx):
     assert ctx.nn_last_units() == -1
     ctx.set_charges(torch_cuda.zeros((0, 4), device="cuda"))
     assert ctx.eval_at_charges_nn().shape == (0, 4)
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_clouds_match_the_oracle(torch_cuda, ctx, nn, ref, seed):
+    """Seeded random sizes, opening parameters, softenings, charge values (zeros included) and clumpy geometries."""
+    rng = np.random.default_rng([61, 99, seed])
+    n = int(rng.integers(1, 30000))
+    theta = float(rng.choice([0.0, 0.5, 2.0, 5.0, 16.0]))
+    eps = float(rng.choice([0.02 * UM, 0.05 * UM]))
+    k = int(rng.integers(1, 6))                                        # clumps
+    centres = rng.uniform(-300 * UM, 300 * UM, (k, 3))
+    x = np.zeros((n, 4), dtype=np.float32)
+    x[:, :3] = centres[rng.integers(0, k, n)] + rng.normal(0, 1, (n, 3)) * rng.uniform(2 * UM, 30 * UM, 3)
+    x[:, 3] = rng.choice([-QE, QE, 2 * QE, 0.0], n, p=[0.4, 0.4, 0.1, 0.1])
+    exp, tree = nn.nn_field(x, eps, theta, ref=ref)
+    got = _gpu_nn(torch_cuda, ctx, x, eps, theta)
+    what = "seed %d: n=%d theta=%g eps=%g clumps=%d" % (seed, n, theta, eps, k)
+    if n > 1 and np.abs(exp).max() > 0:
+        assert_parity(got, exp, what)
+    assert ctx.nn_last_units() == nn.units(tree, theta, n), what
