@@ -160,7 +160,7 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
         const float4 p = x[perm[i]];
         low = nn_ordered(ax == 0 ? p.x : (ax == 1 ? p.y : p.z));
     }
-    keys[i] = ((u64k)a << 32) | (u64k)low;
+    keys[i] = ((u64k)(a / LEAF) << 32) | (u64k)low; /* segment starts are multiples of LEAF: fewer key bits to sort */
 }
 
 /* one CTA per leaf: sorted copy (plain, padded) + blocked copy with header + bounding box + the two pseudo-particles */
@@ -455,8 +455,8 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     const long long far_cap = ceil_div(2 * (n_leaf + n_super), LEAF); /* far blocks a tile can need at most */
     int levels = 0;
     while ((1LL << levels) < n_leaf) ++levels;
-    int nbits = 1;
-    while ((1LL << nbits) <= n) ++nbits;
+    int nbits = 1; /* bits of a segment's leaf index */
+    while ((1LL << nbits) <= n_leaf) ++nbits;
 
     int rc = OBEM_OK;
     for (int k = 0; k < 2 && rc == OBEM_OK; ++k) {
