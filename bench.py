@@ -404,6 +404,8 @@ def run_ours(args):
     }
     if extras:
         roofline["nbody_only_frac"] = FLOP_PER_INTERACTION * extras["nbody_only"]["Ginteractions_per_s"] / 1e3 / peak
+        # BASELINE.json north_star: "at least 60 % of B200 FP32 peak on the 1M-charge N-body evaluation"
+        roofline["north_star_nbody_target"] = {"frac": 0.60, "met": bool(roofline["nbody_only_frac"] >= 0.60)}
         roofline["frac_of_measured_ffma2_peak"] = (achieved / extras["fp32_probe_tflops"]["FFMA2"]
                                                    if extras["fp32_probe_tflops"]["FFMA2"] else None)
 
