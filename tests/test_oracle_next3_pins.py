@@ -217,3 +217,27 @@ def test_t9_sum_wrapper_and_gauss_flux(ref):
     area = 0.5 * np.linalg.norm(np.cross(f64[:, 1] - f64[:, 0], f64[:, 2] - f64[:, 0]), axis=1)
     q = float(np.sum(sigma.astype(np.float64) * area))
     assert abs(flux - q / EPS0) <= 1e-6 * np.sum(np.abs(sigma) * area) / EPS0
+
+
+def test_t10_rectangle_on_axis_potential_closed_form(ref):
+    """phi(h) above the centre of a uniformly charged 2a x 2b rectangle, by direct integration over one quadrant:
+    phi = sigma/(4 pi eps0) * 4 [ a asinh(b / sqrt(a^2 + h^2)) + b asinh(a / sqrt(b^2 + h^2)) - h atan(ab / (h R)) ],
+    R = sqrt(a^2 + b^2 + h^2).  Exact for the exact integrals at any h; the 7-point sum reaches it to 1e-6 from 3 cells up."""
+    a, b, sigma = 50 * UM, 40 * UM, 3e-6
+    tris = _rect_mesh(a, b, 16, 16).astype(np.float32)
+    cell = 2 * a / 16
+    a32, b32 = float(-tris[..., 0].min()), float(-tris[..., 1].min())
+    hs = cell * np.array([0.01, 0.1, 1.0, 3.0, 10.0, 100.0])
+    pts = _pad4(np.stack([np.zeros_like(hs), np.zeros_like(hs), hs], 1))
+    sig = np.full(len(tris), sigma, np.float32)
+    h = pts[:, 2].astype(np.float64)
+    s32 = float(np.float32(sigma))
+    big_r = np.sqrt(a32 ** 2 + b32 ** 2 + h ** 2)
+    quadrant = (a32 * np.arcsinh(b32 / np.sqrt(a32 ** 2 + h ** 2)) + b32 * np.arcsinh(a32 / np.sqrt(b32 ** 2 + h ** 2))
+                - h * np.arctan(a32 * b32 / (h * big_r)))
+    phi = s32 / (4 * np.pi * EPS0) * 4 * quadrant
+    exact = ref.eval_panels_analytic(tris, sig, pts)
+    assert np.allclose(exact[:, 3], phi, rtol=2e-13, atol=0)
+    _, quad = ref.eval_field(verts=tris, sigma=sig, targets=pts, flags=ref.PANELS)
+    assert np.allclose(quad[3:, 3], phi[3:], rtol=1e-6, atol=0)          # h >= 3 cells
+    assert abs(quad[0, 3] / phi[0] - 1) > 1e-4                            # and not at a hundredth of a cell
