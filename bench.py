@@ -110,7 +110,55 @@ def parse_args():
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-next", action="store_true", help="skip the supplementary timings of the adjacent steps")
+    ap.add_argument("--dry-run-ranks", action="store_true",
+                    help="CPU-only check of the multi-rank plumbing (launcher, gloo all-gather of the charge slices, "
+                         "one JSON line from rank 0); no CUDA, no timing claim")
     return ap.parse_args()
+
+
+def launch_ranks(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun around it: start the N ranks ourselves (one process per
+    GPU, rendezvous on 127.0.0.1) and return their exit code.  Fails loudly when fewer than N devices are visible."""
+    import socket
+    if not args.dry_run_ranks:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            print("bench.py: --gpus %d asked for, %d CUDA device(s) visible -- refusing to run fewer ranks than asked"
+                  % (args.gpus, have), file=sys.stderr)
+            return 2
+    sock = socket.socket()
+    sock.bind(("127.0.0.1", 0))
+    port = sock.getsockname()[1]
+    sock.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
+def run_dry_ranks(args) -> int:
+    """The N > 1 host logic without a GPU (tests/test_bench_launcher.py): every rank owns a slice of config 1's
+    charges, all-gathers the full array over gloo (the one exchange of a time step), checks it, and rank 0 prints a
+    line with the rank count it really ran with."""
+    import torch
+    import torch.distributed as dist
+    rank, world, _ = dist_env()
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE is %d" % (args.gpus, world))
+    dist.init_process_group("gloo")
+    wl = W.make_workload(1)
+    n = wl.n_charges
+    first, count = shard_range(n, world, rank)
+    full = all_gather_charges(torch.from_numpy(wl.xyzq[first:first + count].copy()), n)
+    ok = torch.tensor([1 if np.array_equal(full.numpy(), wl.xyzq) else 0])
+    dist.all_reduce(ok, op=dist.ReduceOp.MIN)
+    dist.barrier()
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "metric": METRIC, "value": None, "unit": UNIT, "n_gpus": world,
+                          "scaling": "strong", "gather_ok": bool(ok.item()),
+                          "config": {"workload": "config 1 charges, gloo on CPU: plumbing only"}}), flush=True)
+    dist.destroy_process_group()
+    return 0 if ok.item() else 1
 
 
 def dist_env():
@@ -224,6 +272,8 @@ def run_ours(args):
     import torch.distributed as dist
 
     rank, world, local = dist_env()
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but the launcher started %d rank(s)" % (args.gpus, world))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -375,6 +425,23 @@ def run_ours(args):
         extras = {"nbody_only": {"s": t_nb, "Ginteractions_per_s": n * (n - 1) / t_nb / 1e9},
                   "panels_only": {"s": t_pn, "Ginteractions_per_s": 7 * npan * n / t_pn / 1e9},
                   "fp32_probe_tflops": {"FFMA": probe(0), "FFMA2": probe(1)}}
+        # the same charges in the order the method produces them (electron-ion pairs: signs
+        # interleaved; workloads.pair_creation_order = a seeded permutation): set_charges + N-body launch
+        d_xp = torch.from_numpy(W.pair_creation_order(wl).xyzq).to(dev)
+        t_set = timed(lambda: ctx.set_charges(d_xp))
+        t_nbp = timed(lambda: ctx.eval_at_charges(out=out, flags=api.NBODY))
+        t_eo = timed(lambda: ctx.eval_at_charges(out=out, flags=api.NBODY | api.NO_PHI))
+        extras["nbody_only_pair_order"] = {"s": t_nbp, "Ginteractions_per_s": n * (n - 1) / t_nbp / 1e9,
+                                           "set_charges_s": t_set, "vs_species_order": t_nbp / t_nb - 1.0}
+        extras["nbody_only_E_only"] = {"s": t_eo, "Ginteractions_per_s": n * (n - 1) / t_eo / 1e9,
+                                       "what": "OBEM_NBODY | OBEM_NO_PHI on the pair-ordered charges (11 packed "
+                                               "instructions per interaction pair instead of 12)"}
+        if not args.no_next:
+            t_trkp = timed(lambda: ctx.eval_at_charges_partners(flags=api.NBODY))
+            extras["nbody_with_partners_pair_order"] = {"s": t_trkp, "overhead_vs_nbody_only_pair_order":
+                                                        t_trkp / t_nbp - 1.0}
+        ctx.set_charges(d_x)
+        del d_xp
 
     # ---- supplementary, N = 1 only: the adjacent steps, each against its own roofline ----
     if world == 1 and not args.no_next:
@@ -391,9 +458,10 @@ def run_ours(args):
     eval_s = float(np.mean(eval_ms)) * 1e-3
     achieved = FLOP_PER_INTERACTION * my_inter / eval_s / 1e12
     alg_bytes = 16 * n + 128 * npan + 16 * count + 16 * count                 # sources once, targets in, results out
+    traffic, traffic_src = recorded_traffic(args.config) if world == 1 else (None, "not recorded for N > 1")
     roofline = {
         "bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-        "traffic": TRAFFIC_BYTES_PER_LAUNCH if world == 1 and args.config == 3 else None,
+        "traffic": traffic, "traffic_source": traffic_src,
         "kernel": "obem_eval_kernel: one evaluation = its two launches (charges, then panels) + fix-up / repair "
                   "(< 0.1 %), between CUDA events on the launch stream",
         "peak_source": "derived: %d SMs x %d FP32 lanes x 2 flop x clocks.max.sm %.0f MHz (DESIGN.md); "
@@ -404,6 +472,8 @@ def run_ours(args):
     }
     if extras:
         roofline["nbody_only_frac"] = FLOP_PER_INTERACTION * extras["nbody_only"]["Ginteractions_per_s"] / 1e3 / peak
+        roofline["nbody_only_pair_order_frac"] = (FLOP_PER_INTERACTION * extras["nbody_only_pair_order"]
+                                                  ["Ginteractions_per_s"] / 1e3 / peak)
         # BASELINE.json north_star: "at least 60 % of B200 FP32 peak on the 1M-charge N-body evaluation"
         roofline["north_star_nbody_target"] = {"frac": 0.60, "met": bool(roofline["nbody_only_frac"] >= 0.60)}
         roofline["frac_of_measured_ffma2_peak"] = (achieved / extras["fp32_probe_tflops"]["FFMA2"]
@@ -725,16 +795,44 @@ def bench_next4(torch, api, ctx, wl, timed, dev):
     return res
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE obem_eval_kernel launch on config 3 (N-body + panels), from
-# the `ncu --set full` captures summarised in profiles/r01e_summary.md (one launch per source section):
-# N-body launch 33.80 MB read + 0.71 MB written, panel launch 43.51 MB read + 0.16 MB written.
-TRAFFIC_BYTES_PER_LAUNCH = 33800000 + 710400 + 43510000 + 162000
+def kernel_source_hash() -> str:
+    """sha256 over the sources of the evaluation kernels: ties a recorded ncu figure to the code it was captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("obem.cu", "obem_internal.cuh"):
+        with open(os.path.join(ROOT, "paper_2110_09214_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def recorded_traffic(cfg: int):
+    """`roofline.traffic` cannot be measured inside this process (DRAM counters need ncu), so it is a RECORDED figure:
+    profiles/r02_traffic.json holds dram__bytes_read.sum + dram__bytes_write.sum per evaluation from the committed
+    `ncu --set full` capture, with the hash of the kernel sources it was taken on.  If the sources changed since,
+    the figure is stale and null is reported instead of a wrong number."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        with open(path) as f:
+            rec = json.load(f)
+        ent = rec["configs"].get(str(cfg))
+        if ent is None:
+            return None, "no capture recorded for config %d in profiles/r02_traffic.json" % cfg
+        if rec["kernel_source_hash"] != kernel_source_hash():
+            return None, "stale: profiles/r02_traffic.json was captured on kernel sources %s, these are %s" % (
+                rec["kernel_source_hash"], kernel_source_hash())
+        return ent["bytes_per_evaluation"], "recorded, not measured live: %s (%s)" % (ent["capture"], path[len(ROOT) + 1:])
+    except Exception as e:  # noqa: BLE001
+        return None, "no record: %s" % e
 
 
 def main():
     args = parse_args()
     if args.impl == "reference":
-        return run_reference(args)
+        return run_reference(args)      # rank 0 alone times the oracle; the other ranks of a torchrun exit 0
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return launch_ranks(args)
+    if args.dry_run_ranks:
+        return run_dry_ranks(args)
     return run_ours(args)
 
 

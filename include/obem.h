@@ -59,6 +59,11 @@ typedef enum obem_status {
 #define OBEM_NBODY 1u  /* Eq (3.8), sources = the charges of obem_set_charges              */
 #define OBEM_PANELS 2u /* Eq (2.13)/(2.14), sources = the panels of obem_set_panels         */
 #define OBEM_PANELS_EXACT 4u /* with OBEM_PANELS: exact cell integrals near the target, see obem_set_near_field */
+#define OBEM_NO_PHI 8u /* E only: Eq (3.8) and (2.14) are field sums and the integrators read only E (PAPER.md:274,
+                          :302-306); the phi lane of the result is written as 0 and one packed instruction of 12 per
+                          interaction is saved.  E is bit-identical to the E + phi evaluation.  Accepted by
+                          obem_eval_at_charges[_range] and obem_eval_at_points; not with OBEM_PANELS_EXACT, the
+                          partner by-product or the NN approximation (OBEM_EINVAL).  The steppers use it. */
 
 /* Create a context on CUDA device `device`.  Queries the SM count and sizes the persistent grid.
  * *out is NULL on failure. */
@@ -68,7 +73,10 @@ int obem_create(obem_ctx** out, int device);
 int obem_destroy(obem_ctx* c);
 
 /* Pre-allocate library-owned buffers for up to n_charges charges and n_panels panels, so that later
- * set_* calls never allocate (and therefore never synchronise).  Optional. */
+ * set_* calls never allocate (and therefore never synchronise).  Optional.  A capacity that is already
+ * large enough is left alone; one that has to GROW is re-allocated and the set it held is discarded:
+ * obem_n_charges / obem_n_panels go back to -1 and an evaluation that needs that set returns OBEM_ESTATE
+ * until it is set again.  Call it before the first set_*. */
 int obem_reserve(obem_ctx* c, int64_t n_charges, int64_t n_panels);
 
 /* Softening lengths in metres, >= 0 and finite.  eps_pp: charge-charge sum (reading A2; 0 = Eq 3.8
@@ -91,7 +99,11 @@ int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int
  * (else OBEM_EINVAL; OBEM_ESTATE if no panels were ever set). */
 int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cuda_stream);
 
-/* Charges (Eq 3.8's particles): d_xyzq [n][4] fp32 = x, y, z [m], q [C].  Replaces any earlier set. */
+/* Charges (Eq 3.8's particles): d_xyzq [n][4] fp32 = x, y, z [m], q [C], n < 2^31 - 256.  Replaces any
+ * earlier set.  Any storage order is as fast as any other: the library keeps its copy of the sources
+ * stably sorted by q ("class order": an avalanche creates electrons and ions in pairs, PAPER.md:195-199,
+ * so the caller's array interleaves the signs), which makes its 256-source blocks weight-uniform; every
+ * index the API takes or returns (ranges, partners, output rows) is the CALLER's. */
 int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_stream);
 
 /* E and phi at the charges themselves: d_out [n][4] fp32 = Ex, Ey, Ez [V/m], phi [V].
@@ -99,8 +111,9 @@ int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_str
  * an EMPTY set contributes 0; a flag whose sources were NEVER set gives OBEM_ESTATE. */
 int obem_eval_at_charges(obem_ctx* c, float* d_out, unsigned flags, void* cuda_stream);
 
-/* Same, for the contiguous slice [first, first+count) of the charges only: d_out [count][4].
- * This is the multi-GPU sharding unit (targets sharded across ranks, sources replicated). */
+/* Same, for the contiguous slice [first, first+count) of the charges (the caller's indices) only:
+ * d_out [count][4], row i = charge first + i.  This is the multi-GPU sharding unit (targets sharded
+ * across ranks, sources replicated). */
 int obem_eval_at_charges_range(obem_ctx* c, int64_t first, int64_t count, float* d_out,
                                unsigned flags, void* cuda_stream);
 

@@ -14,6 +14,7 @@ from . import build as _build
 NBODY = 1   # OBEM_NBODY  -- Eq (3.8)
 PANELS = 2  # OBEM_PANELS -- Eq (2.13)/(2.14)
 PANELS_EXACT = 4  # OBEM_PANELS_EXACT -- with PANELS: closed-form cell integrals near the target (NEXT-3)
+NO_PHI = 8  # OBEM_NO_PHI -- E only (Eq 3.8 / 2.14 are field sums); the phi lane of the result is 0
 
 _c_fp = ctypes.c_void_p  # device or host float* passed as an address
 _i64 = ctypes.c_int64

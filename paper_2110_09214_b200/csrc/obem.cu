@@ -23,6 +23,10 @@
  */
 #include <new>
 
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_select.cuh>
+#include <thrust/iterator/counting_iterator.h>
+
 #include "obem_internal.cuh"
 
 namespace {
@@ -111,7 +115,7 @@ struct EvalParams {
     long long ntiles;     /* ceil(nt / TT)                                                               */
     long long U;          /* work units = ntiles * nblk                                                  */
     float4* out;          /* [nt]                                                                        */
-    float4* ws;           /* [grid][2][TT] partial sums of split tiles                                   */
+    double* ws;           /* [grid][2][TT_MAX][4] fp64 partial sums (Ex, Ey, Ez, phi) of split tiles      */
     long long self_first; /* >= 0: target i IS point source (self_first + i) of sec[0] and is excluded
                              from its own sum by index (reading A3); -1: no exclusion                    */
     float2* trk_out;      /* TRACK: [nt] (min softened r2 over opposite-sign sources, its block index as int bits) */
@@ -130,8 +134,16 @@ struct EvalParams {
     /* appended (the point kernel's parameter offsets stay as they were): geometry of THIS launch for the fix-up and
      * repair kernels -- targets per thread / per tile, and the stride of a workspace slot */
     int tpt, tt, ws_stride;
+    /* class order (set_charges sorts the sources by q): the targets of an evaluation at the charges are taken in the
+     * sources' order, and their results are scattered to the caller's order on write */
+    const int* out_idx;   /* != NULL: the result of target i goes to out[out_idx[i]] (trk_out likewise)            */
+    const int* spos;      /* != NULL: target i IS point source spos[i] of sec[0] (ascending in i);
+                             NULL: it is source self_first + i                                                   */
 };
 constexpr unsigned BAD_CAP = 1u << 20;
+/* dynamic shared memory of the evaluation kernels: their fp64 running sums (acc_flush) */
+constexpr size_t ACC_BYTES_POINTS = (size_t)8 * NPAIR * THREADS * sizeof(double);
+constexpr size_t ACC_BYTES_PANELS = (size_t)8 * PANEL_NPAIR * THREADS * sizeof(double);
 
 __device__ __forceinline__ bool all_finite(float a, float b, float c, float d)
 {
@@ -194,11 +206,12 @@ __device__ __forceinline__ float min_nonneg(float a, float b)
 {
     return __int_as_float(min(__float_as_int(a), __float_as_int(b)));
 }
+template <bool PHI>
 __device__ __forceinline__ void item_back(const u64 dx, const u64 dy, const u64 dz, const u64 u, const u64 w,
                                           u64& ax, u64& ay, u64& az, u64& ap)
 {
     const u64 t = mul2(u, w);
-    ap = add2(ap, t);
+    if (PHI) ap = add2(ap, t);
     const u64 u2 = mul2(u, u);
     const u64 sE = mul2(t, u2);
     ax = fma2(sE, dx, ax);
@@ -208,9 +221,10 @@ __device__ __forceinline__ void item_back(const u64 dx, const u64 dy, const u64 
 
 /* One block of SB point sources against the thread's TPT targets (KIND_POINTS).  Unguarded: see the
  * "speculative zero-distance handling" note at obem_repair_kernel. */
+template <bool TRACK, bool PHI>
 __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
-                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR])
+                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
 {
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR; /* work items (source, target pair) per trip */
@@ -226,11 +240,19 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
-                item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+                if (TRACK) { /* as in block_loop_uniform: the block is of one sign (header .y), decided after the block */
+                    float r2l, r2h;
+                    item_front_r2<false>(dX[k], dY[k], dZ[k], U[k], r2l, r2h, X[p], Y[p], Z[p], q[j].x, q[j].y,
+                                         q[j].z, e2);
+                    bm[2 * p] = min_nonneg(bm[2 * p], r2l);
+                    bm[2 * p + 1] = min_nonneg(bm[2 * p + 1], r2h);
+                } else {
+                    item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+                }
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
-                item_back(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
+                item_back<PHI>(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
             }
         }
     }
@@ -240,7 +262,7 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
  * Same for a block whose SB sources all carry the weight w (header): sum_j w f(r_j) = w sum_j f(r_j), so the
  * weight is applied once per block and the body is 12 packed instructions: phi += u, u^2, u^3, E += u^3 d.
  */
-template <bool TRACK>
+template <bool TRACK, bool PHI>
 __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2, const float w,
                                                    const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
@@ -272,7 +294,7 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, p = kk % NPAIR;
-                aP[p] = add2(aP[p], U[kk]);
+                if (PHI) aP[p] = add2(aP[p], U[kk]);
                 const u64 u2 = mul2(U[kk], U[kk]);
                 const u64 u3 = mul2(u2, U[kk]);
                 aX[p] = fma2(u3, dX[kk], aX[p]);
@@ -287,7 +309,7 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
         aX[p] = mul2(aX[p], w2);
         aY[p] = mul2(aY[p], w2);
         aZ[p] = mul2(aZ[p], w2);
-        aP[p] = mul2(aP[p], w2);
+        if (PHI) aP[p] = mul2(aP[p], w2);
     }
 }
 
@@ -307,7 +329,7 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
  * (source, target pair) instead of 13, like a uniform point block.  Softening: r2' += a^2 eps^2 (B.y = a^2).
  * A source of weight 0 is stored as a = 0, b = 1e17: u'^3 underflows to exactly 0, c_phi = 0.
  */
-template <bool HAS_EPS, int NP>
+template <bool HAS_EPS, int NP, bool PHI>
 __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NP],
                                            const u64 (&Y)[NP], const u64 (&Z)[NP], u64 (&aX)[NP],
                                            u64 (&aY)[NP], u64 (&aZ)[NP], u64 (&aP)[NP])
@@ -357,7 +379,7 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
-                aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
+                if (PHI) aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
                 const u64 u2 = mul2(U[kk], U[kk]);
                 const u64 u3 = mul2(u2, U[kk]);
                 aX[p] = fma2(u3, dX[kk], aX[p]);
@@ -371,15 +393,15 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
 /*
  * The rare diagonal block: a block of point sources that contains some of this tile's own targets
  * (evaluation at the charges).  Eq (3.8)'s p != p' is applied BY INDEX: the weight of source j is
- * zeroed for the target whose source index is j.  selfrel[k] = (source index of target slot k) - (first
- * source index of the block); always guarded (d = 0 there).  Simple loop: it runs for TT/SB of the
- * blocks of a tile only.
+ * zeroed for the target whose source index is j.  rel[k] = (source index of target slot k) - (first
+ * source index of the block), or -1 if that target is not in this block; always guarded (d = 0 there).
+ * Simple loop: it runs for ~TT/SB of the blocks of a tile only.
  */
-template <bool TRACK>
+template <bool TRACK, bool PHI>
 __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                              const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                              u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR],
-                                             const long long selfrel0, const int selfrel_stride, float (&bm)[TPT],
+                                             const int (&rel)[TPT], float (&bm)[TPT],
                                              const unsigned negmask, const unsigned posmask)
 {
     const u64 e2 = pk(eps2, eps2);
@@ -400,26 +422,13 @@ __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, co
             } else {
                 item_front<true>(dx, dy, dz, u, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
             }
-            const float wl = (selfrel0 + (long long)(2 * p) * selfrel_stride == j) ? 0.0f : q.w;
-            const float wh = (selfrel0 + (long long)(2 * p + 1) * selfrel_stride == j) ? 0.0f : q.w;
-            item_back(dx, dy, dz, u, pk(wl, wh), aX[p], aY[p], aZ[p], aP[p]);
+            const float wl = (rel[2 * p] == j) ? 0.0f : q.w;
+            const float wh = (rel[2 * p + 1] == j) ? 0.0f : q.w;
+            item_back<PHI>(dx, dy, dz, u, pk(wl, wh), aX[p], aY[p], aZ[p], aP[p]);
         }
     }
 }
 
-__device__ __forceinline__ const float4* unit_src(const EvalParams& P, long long blk)
-{
-    return (blk < P.sec[0].nblk) ? P.sec[0].src + blk * P.sec[0].stride
-                                 : P.sec[1].src + (blk - P.sec[0].nblk) * P.sec[1].stride;
-}
-__device__ __forceinline__ unsigned unit_bytes(const EvalParams& P, long long blk)
-{
-    return (unsigned)((blk < P.sec[0].nblk) ? P.sec[0].stride : P.sec[1].stride) * (unsigned)sizeof(float4);
-}
-
-/* One launch per source section: KIND selects the loops compiled in (P.sec[0] is the section; P.sec[1] is empty).
- * Two instantiations instead of one kernel with both loop families: each hot loop gets its own register
- * allocation (a combined kernel cost the uniform N-body loop 8 extra MOVs per trip, -4 %). */
 /* tile whose unit range [tile_ptr[t], tile_ptr[t+1]) contains u (LIST mode; empty tiles are skipped) */
 __device__ __forceinline__ long long list_tile_of(const long long* __restrict__ tile_ptr, long long ntiles, long long u)
 {
@@ -432,17 +441,98 @@ __device__ __forceinline__ long long list_tile_of(const long long* __restrict__ 
     return lo;
 }
 
-template <int KIND, bool TRACK, bool LIST = false>
+/*
+ * Second accumulation level (a5).  The block sums (fp32, 256 sources or 34 panels) are flushed into per-target
+ * running sums that live in SHARED memory as fp64: acc[(4 slot + component) THREADS + tid].  Why not fp32 registers:
+ * the sources are grouped by sign, so the running sum of a neutral cloud travels to ~50x (config 4: ~200x) its final
+ * value and back, and an fp32 running sum loses that factor times 6e-8 (round 1 measured it: phi 2e-5 rms on config
+ * 1, and config 4's E failed the 2e-5 bar once the class order put ALL electrons first).  In fp64 the flush is exact
+ * to 1e-16, costs 4 DADD per target and block on the otherwise idle FP64 pipe (0.3 % of the block's instructions),
+ * and frees the 32-40 registers the running sums occupied in the hot loops.  What is left of the accumulation error
+ * is the fp32 sum inside one block.
+ */
+template <int NP, bool PHI>
+__device__ __forceinline__ void acc_clear(double* __restrict__ acc)
+{
+#pragma unroll
+    for (int v = 0; v < 8 * NP; ++v)
+        if (PHI || (v & 3) != 3) acc[v * THREADS] = 0.0;
+}
+template <int NP, bool PHI>
+__device__ __forceinline__ void acc_flush(double* __restrict__ acc, const u64 (&aX)[NP], const u64 (&aY)[NP],
+                                          const u64 (&aZ)[NP], const u64 (&aP)[NP])
+{
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        float l, h;
+        double* a = acc + (size_t)(8 * p) * THREADS; /* slots 2p (lo lanes) and 2p + 1 (hi lanes) */
+        upk(aX[p], l, h);
+        a[0 * THREADS] += (double)l;
+        a[4 * THREADS] += (double)h;
+        upk(aY[p], l, h);
+        a[1 * THREADS] += (double)l;
+        a[5 * THREADS] += (double)h;
+        upk(aZ[p], l, h);
+        a[2 * THREADS] += (double)l;
+        a[6 * THREADS] += (double)h;
+        if (PHI) {
+            upk(aP[p], l, h);
+            a[3 * THREADS] += (double)l;
+            a[7 * THREADS] += (double)h;
+        }
+    }
+}
+
+/* End of a CTA's run over (part of) a tile: a tile it covered completely is scaled by k_e and written (scattered
+ * through out_idx if the targets are in class order); a partial run goes to the CTA's workspace slot in fp64. */
+template <int NP, bool PHI>
+__device__ __forceinline__ void run_epilogue(const EvalParams& P, const double* __restrict__ acc, const long long tbase,
+                                             const bool whole, double* __restrict__ wsl)
+{
+#pragma unroll
+    for (int k = 0; k < 2 * NP; ++k) {
+        const double* a = acc + (size_t)(4 * k) * THREADS;
+        const double ex = a[0], ey = a[THREADS], ez = a[2 * THREADS], ph = PHI ? a[3 * THREADS] : 0.0;
+        if (whole) {
+            const long long i = tbase + (long long)k * THREADS;
+            if (i >= P.nt) continue;
+            const long long oi = P.out_idx ? (long long)__ldg(P.out_idx + i) : i;
+            float4 o = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
+            /* a non-finite partial of THIS launch goes to the repair list (once: a later accumulating launch adds to
+             * it without reporting it again) */
+            if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, oi);
+            if (P.accumulate) {
+                const float4 q = P.out[oi];
+                o = make_float4(o.x + q.x, o.y + q.y, o.z + q.z, o.w + q.w);
+            }
+            P.out[oi] = o;
+        } else {
+            double2* w = reinterpret_cast<double2*>(wsl + (size_t)k * THREADS * 4);
+            w[0] = make_double2(ex, ey);
+            w[1] = make_double2(ez, ph);
+        }
+    }
+}
+
+/*
+ * The N-body launch (a3 + a5) and its variants: TRACK (recombination partners, NEXT-2), LIST (the NN approximation's
+ * per-tile source lists, NEXT-4), PHI = false (E only: Eq 3.8 as printed is a field sum, and the
+ * integrators read only E, PAPER.md:302-306 -- one packed instruction of 12 less).  One instantiation per variant:
+ * each hot loop gets its own register allocation.
+ */
+template <bool TRACK, bool LIST, bool PHI>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
 {
-    static_assert(!LIST || (KIND == KIND_POINTS && !TRACK), "LIST mode: point sources, no partner tracking");
-    __shared__ __align__(128) float4 ring[STAGES][KIND == KIND_PANELS ? SBH_P : SBH + 3]; /* stage stride % 64 B == 0 */
+    static_assert(!LIST || !TRACK, "LIST mode: no partner tracking");
+    extern __shared__ __align__(16) double acc_dyn[]; /* [8 NPAIR][THREADS] running sums, fp64 */
+    __shared__ __align__(128) float4 ring[STAGES][SBH + 3]; /* stage stride % 64 B == 0 */
     __shared__ __align__(8) u64 full[STAGES];
     /* TRACK: running (min r2, block) per target slot, updated once per block */
     __shared__ float trk_m[TRACK ? TPT : 1][THREADS];
     __shared__ int trk_b[TRACK ? TPT : 1][THREADS];
 
     const int tid = threadIdx.x;
+    double* const acc = acc_dyn + tid;
     const long long G = gridDim.x, c = blockIdx.x;
     const long long Utot = LIST ? *P.U_dev : P.U;
     const long long u0 = unit_begin(c, Utot, G), u1 = unit_begin(c + 1, Utot, G);
@@ -455,22 +545,17 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
     __syncthreads();
 
     /* producer state (thread 0): next unit to load and its source block */
+    const unsigned bytes = (unsigned)(SBH * sizeof(float4));
+    const float4* const src = LIST ? P.pool : P.sec[0].src;
     long long pu = u0, pblk = LIST ? 0 : u0 % P.nblk;
     if (tid == 0) {
         for (int s = 0; s < STAGES - 1 && pu < u1; ++s) {
-            if (LIST) {
-                mbar_expect_tx(&full[s], (unsigned)(SBH * sizeof(float4)));
-                tma_load_1d(&ring[s][0], P.pool + (long long)P.list[pu] * SBH, (unsigned)(SBH * sizeof(float4)), &full[s]);
-            } else {
-                mbar_expect_tx(&full[s], unit_bytes(P, pblk));
-                tma_load_1d(&ring[s][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[s]);
-            }
+            mbar_expect_tx(&full[s], bytes);
+            tma_load_1d(&ring[s][0], src + (LIST ? (long long)P.list[pu] : pblk) * SBH, bytes, &full[s]);
             ++pu;
             if (++pblk == P.nblk) pblk = 0;
         }
     }
-
-    const float ke = (float)KE_D;
 
     long long u = u0;
     unsigned it = 0; /* units consumed so far by this CTA: stage = it % STAGES, parity = (it / STAGES) & 1 */
@@ -485,8 +570,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
         const long long b0 = u - tile_u0;
         const long long nrun = min(tile_u1 - u, u1 - u);
         const long long tbase = tile * (long long)TT + tid;
-        /* decided here, not after the block loop: tile_u0 / tile_u1 then do not stay live across the hot loops
-         * (measured: -1.1 % on the N-body launch) */
+        /* decided here, not after the block loop: tile_u0 / tile_u1 then do not stay live across the hot loops */
         const bool whole = (b0 == 0 && u + nrun == tile_u1);
 
         u64 X[NPAIR], Y[NPAIR], Z[NPAIR];
@@ -502,9 +586,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             Y[p] = pk_keep(va ? __ldg(ta + 1) : 0.f, vb ? __ldg(tb + 1) : 0.f);
             Z[p] = pk_keep(va ? __ldg(ta + 2) : 0.f, vb ? __ldg(tb + 2) : 0.f);
         }
-        u64 RX[NPAIR], RY[NPAIR], RZ[NPAIR], RP[NPAIR];
-#pragma unroll
-        for (int p = 0; p < NPAIR; ++p) RX[p] = RY[p] = RZ[p] = RP[p] = 0ull;
+        acc_clear<NPAIR, PHI>(acc);
         unsigned negmask = 0u, posmask = 0u; /* TRACK: bit k set = target slot k is negative / positive */
         if (TRACK) {
 #pragma unroll
@@ -518,8 +600,15 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             }
         }
 
-        /* source-index range of this tile's own targets inside sec[0] (evaluation at the charges) */
-        const long long self_lo = (P.self_first >= 0) ? P.self_first + tile * (long long)TT : -1;
+        /* blocks of sec[0] that hold this tile's own targets (evaluation at the charges): the targets are in the
+         * sources' order, so these are the blocks [dlo, dhi] of its first and last target -- exactly (spos == NULL:
+         * the whole set) or as a hull that is refined per block (a sub-range straddles the class boundaries) */
+        long long dlo = 0, dhi = -1;
+        if (P.self_first >= 0) {
+            const long long t0 = tile * (long long)TT, t1 = min(t0 + TT, P.nt) - 1;
+            dlo = (P.spos ? (long long)__ldg(P.spos + t0) : P.self_first + t0) / SB;
+            dhi = (P.spos ? (long long)__ldg(P.spos + t1) : P.self_first + t1) / SB;
+        }
 
         int next_blk = LIST ? __ldg(P.list + u) : 0;
         for (long long r = 0; r < nrun; ++r, ++it) {
@@ -528,14 +617,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
             if (tid == 0 && pu < u1) {
                 const int ps = (it + STAGES - 1) % STAGES;
-                if (LIST) {
-                    mbar_expect_tx(&full[ps], (unsigned)(SBH * sizeof(float4)));
-                    tma_load_1d(&ring[ps][0], P.pool + (long long)P.list[pu] * SBH, (unsigned)(SBH * sizeof(float4)),
-                                &full[ps]);
-                } else {
-                    mbar_expect_tx(&full[ps], unit_bytes(P, pblk));
-                    tma_load_1d(&ring[ps][0], unit_src(P, pblk), unit_bytes(P, pblk), &full[ps]);
-                }
+                mbar_expect_tx(&full[ps], bytes);
+                tma_load_1d(&ring[ps][0], src + (LIST ? (long long)P.list[pu] : pblk) * SBH, bytes, &full[ps]);
                 ++pu;
                 if (++pblk == P.nblk) pblk = 0;
             }
@@ -547,89 +630,65 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             for (int p = 0; p < NPAIR; ++p) aX[p] = aY[p] = aZ[p] = aP[p] = 0ull;
             const float eps2 = P.sec[0].eps2;
             const float4* sblk = &ring[st][1];
-            if (KIND == KIND_PANELS) {
-                if (eps2 != 0.f) panel_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
-                else panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            const float blkw = ring[st][0].x; /* header: common weight of the block, or NaN */
+            float bm[TPT];
+            unsigned elig = 0xffu; /* TRACK: target slots for which bm counts (the slow loop masks per source) */
+            if (TRACK) {
+#pragma unroll
+                for (int k = 0; k < TPT; ++k) bm[k] = __int_as_float(0x7f800000);
+            }
+            bool diag = (!LIST || blk < P.list_self_blocks) && blk >= dlo && blk <= dhi;
+            if (diag && P.spos) { /* CTA-uniform branch: inside the hull, does any target really live in blk? */
+                int mine = 0;
+#pragma unroll
+                for (int k = 0; k < TPT; ++k) {
+                    const long long i = tbase + (long long)k * THREADS;
+                    mine |= (i < P.nt && (long long)(__ldg(P.spos + i) / SB) == blk) ? 1 : 0;
+                }
+                diag = __syncthreads_or(mine) != 0;
+            }
+            /* TRACK: sign of the block's sources (header .y: +1, -1, 0 = all zero weights; NaN = mixed signs,
+             * which after the class sort happens only in the <= 2 blocks that straddle a sign boundary) */
+            const float blks = TRACK ? ring[st][0].y : 0.f;
+            if (diag || (TRACK && !(blks == blks))) {
+                int rel[TPT];
+#pragma unroll
+                for (int k = 0; k < TPT; ++k) {
+                    const long long i = tbase + (long long)k * THREADS;
+                    long long rr = -1;
+                    if (diag && i < P.nt) rr = (P.spos ? (long long)__ldg(P.spos + i) : P.self_first + i) - blk * SB;
+                    rel[k] = (rr >= 0 && rr < SB) ? (int)rr : -1;
+                }
+                self_block_loop<TRACK, PHI>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, rel, bm, negmask, posmask);
+            } else if (blkw == blkw) {
+                block_loop_uniform<TRACK, PHI>(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP, bm);
+                elig = (blkw > 0.f) ? negmask : ((blkw < 0.f) ? posmask : 0u);
             } else {
-                const float blkw = ring[st][0].x; /* header: common weight of the block, or NaN */
-                float bm[TPT];
-                unsigned elig = 0xffu; /* TRACK: target slots for which bm counts (the slow loop masks per source) */
-                if (TRACK) {
+                block_loop<TRACK, PHI>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, bm);
+                elig = (blks > 0.f) ? negmask : ((blks < 0.f) ? posmask : 0u);
+            }
+            if (TRACK) {
 #pragma unroll
-                    for (int k = 0; k < TPT; ++k) bm[k] = __int_as_float(0x7f800000);
-                }
-                const bool diag = self_lo >= 0 && (!LIST || blk < P.list_self_blocks) && blk * SB < self_lo + TT &&
-                                  (blk + 1) * SB > self_lo;
-                if (diag || (TRACK && !(blkw == blkw))) {
-                    self_block_loop<TRACK>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP,
-                                           diag ? self_lo + tid - blk * SB : -(1LL << 40), THREADS, bm, negmask, posmask);
-                } else if (blkw == blkw) {
-                    block_loop_uniform<TRACK>(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP, bm);
-                    elig = (blkw > 0.f) ? negmask : ((blkw < 0.f) ? posmask : 0u);
-                } else {
-                    block_loop(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
-                }
-                if (TRACK) {
-#pragma unroll
-                    for (int k = 0; k < TPT; ++k) {
-                        if (((elig >> k) & 1u) && bm[k] < trk_m[k][tid]) {
-                            trk_m[k][tid] = bm[k];
-                            trk_b[k][tid] = (int)blk;
-                        }
+                for (int k = 0; k < TPT; ++k) {
+                    if (((elig >> k) & 1u) && bm[k] < trk_m[k][tid]) {
+                        trk_m[k][tid] = bm[k];
+                        trk_b[k][tid] = (int)blk;
                     }
                 }
             }
-            /* second accumulation level: flush the block sums into the running sums */
-#pragma unroll
-            for (int p = 0; p < NPAIR; ++p) {
-                RX[p] = add2(RX[p], aX[p]);
-                RY[p] = add2(RY[p], aY[p]);
-                RZ[p] = add2(RZ[p], aZ[p]);
-                RP[p] = add2(RP[p], aP[p]);
-            }
+            acc_flush<NPAIR, PHI>(acc, aX, aY, aZ, aP);
         }
 
-        float4* wsl = P.ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT + tid;
-#pragma unroll
-        for (int p = 0; p < NPAIR; ++p) {
-            float4 a, b;
-            upk(RX[p], a.x, b.x);
-            upk(RY[p], a.y, b.y);
-            upk(RZ[p], a.z, b.z);
-            upk(RP[p], a.w, b.w);
-            if (whole) {
-                const long long i0 = tbase + (2 * p) * THREADS, i1 = i0 + THREADS;
-                if (i0 < P.nt) {
-                    float4 o = make_float4(ke * a.x, ke * a.y, ke * a.z, ke * a.w);
-                    if (P.accumulate) {
-                        const float4 h = P.out[i0];
-                        o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
-                    }
-                    P.out[i0] = o;
-                    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i0);
-                }
-                if (i1 < P.nt) {
-                    float4 o = make_float4(ke * b.x, ke * b.y, ke * b.z, ke * b.w);
-                    if (P.accumulate) {
-                        const float4 h = P.out[i1];
-                        o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
-                    }
-                    P.out[i1] = o;
-                    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i1);
-                }
-            } else {
-                wsl[(2 * p) * THREADS] = a;
-                wsl[(2 * p + 1) * THREADS] = b;
-            }
-        }
+        const size_t slot = (size_t)c * 2 + (u == u0 ? 0 : 1);
+        run_epilogue<NPAIR, PHI>(P, acc, tbase, whole, P.ws + (slot * TT_MAX + tid) * 4);
         if (TRACK) {
-            float2* tw = P.trk_ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT + tid;
+            float2* tw = P.trk_ws + slot * TT + tid;
 #pragma unroll
             for (int k = 0; k < TPT; ++k) {
                 const float2 v = make_float2(trk_m[k][tid], __int_as_float(trk_b[k][tid]));
                 const long long i = tbase + (long long)k * THREADS;
                 if (whole) {
-                    if (i < P.nt) P.trk_out[i] = v;
+                    if (i < P.nt) P.trk_out[P.out_idx ? (long long)__ldg(P.out_idx + i) : i] = v;
                 } else {
                     tw[k * THREADS] = v;
                 }
@@ -640,18 +699,19 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
 }
 
 /*
- * The panel launch (a4 + a5): the same persistent stream-K structure as obem_eval_kernel<KIND_PANELS>, as a kernel of
- * its own with NP target pairs per thread (tile = THREADS * 2 NP targets).  No self term, no partner tracking, no
- * lists: panels only.
+ * The panel launch (a4 + a5): the same persistent stream-K structure as a kernel of its own with NP target pairs per
+ * thread (tile = THREADS * 2 NP targets).  No self term, no partner tracking, no lists: panels only.
  */
-template <int NP>
+template <int NP, bool PHI>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_panels_kernel(const EvalParams P)
 {
     constexpr int TTP = THREADS * 2 * NP;
+    extern __shared__ __align__(16) double acc_dyn[]; /* [8 NP][THREADS] running sums, fp64 */
     __shared__ __align__(128) float4 ring[STAGES][SBH_P];
     __shared__ __align__(8) u64 full[STAGES];
 
     const int tid = threadIdx.x;
+    double* const acc = acc_dyn + tid;
     const long long G = gridDim.x, c = blockIdx.x;
     const long long u0 = unit_begin(c, P.U, G), u1 = unit_begin(c + 1, P.U, G);
     if (u0 >= u1) return;
@@ -671,7 +731,6 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_panels_kernel(const
             if (++pblk == P.nblk) pblk = 0;
         }
     }
-    const float ke = (float)KE_D;
     const float eps2 = P.sec[0].eps2;
     long long u = u0;
     unsigned it = 0;
@@ -692,9 +751,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_panels_kernel(const
             Y[p] = pk_keep(va ? __ldg(ta + 1) : 0.f, vb ? __ldg(tb + 1) : 0.f);
             Z[p] = pk_keep(va ? __ldg(ta + 2) : 0.f, vb ? __ldg(tb + 2) : 0.f);
         }
-        u64 RX[NP], RY[NP], RZ[NP], RP[NP];
-#pragma unroll
-        for (int p = 0; p < NP; ++p) RX[p] = RY[p] = RZ[p] = RP[p] = 0ull;
+        acc_clear<NP, PHI>(acc);
 
         for (long long r = 0; r < nrun; ++r, ++it) {
             __syncthreads(); /* everyone is done with the stage consumed in the previous iteration */
@@ -711,44 +768,12 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_panels_kernel(const
 #pragma unroll
             for (int p = 0; p < NP; ++p) aX[p] = aY[p] = aZ[p] = aP[p] = 0ull;
             const float4* sblk = &ring[st][1];
-            if (eps2 != 0.f) panel_loop<true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
-            else panel_loop<false>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
-#pragma unroll
-            for (int p = 0; p < NP; ++p) { /* second accumulation level */
-                RX[p] = add2(RX[p], aX[p]);
-                RY[p] = add2(RY[p], aY[p]);
-                RZ[p] = add2(RZ[p], aZ[p]);
-                RP[p] = add2(RP[p], aP[p]);
-            }
+            if (eps2 != 0.f) panel_loop<true, NP, PHI>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            else panel_loop<false, NP, PHI>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP);
+            acc_flush<NP, PHI>(acc, aX, aY, aZ, aP);
         }
-
-        float4* wsl = P.ws + ((size_t)c * 2 + (u == u0 ? 0 : 1)) * TT_MAX + tid;
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-            float4 a, b;
-            upk(RX[p], a.x, b.x);
-            upk(RY[p], a.y, b.y);
-            upk(RZ[p], a.z, b.z);
-            upk(RP[p], a.w, b.w);
-            if (whole) {
-                const long long idx[2] = {tbase + (2 * p) * THREADS, tbase + (2 * p + 1) * THREADS};
-                const float4 v[2] = {a, b};
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    if (idx[h] >= P.nt) continue;
-                    float4 o = make_float4(ke * v[h].x, ke * v[h].y, ke * v[h].z, ke * v[h].w);
-                    if (P.accumulate) {
-                        const float4 q = P.out[idx[h]];
-                        o = make_float4(o.x + q.x, o.y + q.y, o.z + q.z, o.w + q.w);
-                    }
-                    P.out[idx[h]] = o;
-                    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, idx[h]);
-                }
-            } else {
-                wsl[(2 * p) * THREADS] = a;
-                wsl[(2 * p + 1) * THREADS] = b;
-            }
-        }
+        const size_t slot = (size_t)c * 2 + (u == u0 ? 0 : 1);
+        run_epilogue<NP, PHI>(P, acc, tbase, whole, P.ws + (slot * TT_MAX + tid) * 4);
         u += nrun;
     }
 }
@@ -784,56 +809,60 @@ __device__ __forceinline__ long long cta_of(long long u, long long U, long long 
     return c;
 }
 
-/* Tiles that were split between CTAs: sum their partials (fixed order, fp64), scale, write. */
+/* Tiles that were split between CTAs: sum their partials (fixed order, fp64), scale, write.  One CTA per (tile,
+ * target slot k): thread t owns target tile * tt + k * THREADS + t.  The unit ranges of the CTAs that share the tile
+ * are formed once per CTA (one 64-bit division per thread, none in the summation loop). */
 __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P, const int G)
 {
+    extern __shared__ long long cta_u0[]; /* [cB - cA + 2] first unit of CTAs cA .. cB + 1 */
     const long long tile = blockIdx.x;
+    const int k = blockIdx.y;
     const bool LIST = P.list != nullptr;
     const long long Utot = LIST ? *P.U_dev : P.U;
     const long long uA = LIST ? P.tile_ptr[tile] : tile * P.nblk;
     const long long uB = (LIST ? P.tile_ptr[tile + 1] : uA + P.nblk) - 1;
     const int tid = threadIdx.x;
+    const long long i = tile * (long long)P.tt + (long long)k * THREADS + tid;
     if (uB < uA) { /* LIST: a tile with no unit at all */
-        for (int k = 0; k < P.tpt; ++k) {
-            const long long i = tile * (long long)P.tt + (long long)k * THREADS + tid;
-            if (i < P.nt && !P.accumulate) P.out[i] = make_float4(0.f, 0.f, 0.f, 0.f);
-        }
+        if (i < P.nt && !P.accumulate) P.out[P.out_idx ? (long long)P.out_idx[i] : i] = make_float4(0.f, 0.f, 0.f, 0.f);
         return;
     }
     const long long cA = cta_of(uA, Utot, G), cB = cta_of(uB, Utot, G);
     if (cA == cB) return; /* one CTA had the whole tile and wrote it directly */
-    for (int k = 0; k < P.tpt; ++k) {
-        const long long i = tile * (long long)P.tt + (long long)k * THREADS + tid;
-        if (i >= P.nt) continue;
-        double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
-        float tm = __int_as_float(0x7f800000);
-        int tb = -1;
-        for (long long c = cA; c <= cB; ++c) {
-            const long long c0 = unit_begin(c, Utot, G), c1 = unit_begin(c + 1, Utot, G);
-            if (c0 >= c1) continue;
-            const int slot = (c0 >= uA && c0 <= uB) ? 0 : 1; /* the CTA's range STARTS inside this tile */
-            if (P.trk_out) { /* CTAs in ascending block order: strict < keeps the lowest block on ties */
-                const float2 t = P.trk_ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
-                if (t.x < tm) {
-                    tm = t.x;
-                    tb = __float_as_int(t.y);
-                }
+    for (long long c = cA + tid; c <= cB + 1; c += THREADS) cta_u0[c - cA] = unit_begin(c, Utot, G);
+    __syncthreads();
+    if (i >= P.nt) return;
+    double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
+    float tm = __int_as_float(0x7f800000);
+    int tb = -1;
+    for (long long c = cA; c <= cB; ++c) {
+        const long long c0 = cta_u0[c - cA], c1 = cta_u0[c - cA + 1];
+        if (c0 >= c1) continue;
+        const int slot = (c0 >= uA && c0 <= uB) ? 0 : 1; /* the CTA's range STARTS inside this tile */
+        if (P.trk_out) { /* CTAs in ascending block order: strict < keeps the lowest block on ties */
+            const float2 t = P.trk_ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
+            if (t.x < tm) {
+                tm = t.x;
+                tb = __float_as_int(t.y);
             }
-            const float4 v = P.ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
-            ex += (double)v.x;
-            ey += (double)v.y;
-            ez += (double)v.z;
-            ph += (double)v.w;
         }
-        float4 o = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
-        if (P.accumulate) {
-            const float4 h = P.out[i];
-            o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
-        }
-        P.out[i] = o;
-        if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, i);
-        if (P.trk_out) P.trk_out[i] = make_float2(tm, __int_as_float(tb));
+        const double2* v =
+            reinterpret_cast<const double2*>(P.ws + (((size_t)c * 2 + slot) * TT_MAX + (size_t)k * THREADS + tid) * 4);
+        const double2 v0 = v[0], v1 = v[1];
+        ex += v0.x;
+        ey += v0.y;
+        ez += v1.x;
+        ph += v1.y;
     }
+    const long long oi = P.out_idx ? (long long)P.out_idx[i] : i;
+    float4 o = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
+    if (!all_finite(o.x, o.y, o.z, o.w)) report_bad(P, oi);
+    if (P.accumulate) {
+        const float4 h = P.out[oi];
+        o = make_float4(o.x + h.x, o.y + h.y, o.z + h.z, o.w + h.w);
+    }
+    P.out[oi] = o;
+    if (P.trk_out) P.trk_out[oi] = make_float2(tm, __int_as_float(tb));
 }
 
 /*
@@ -843,7 +872,8 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
  * writes the partner's true distance and index; ties go to the smallest index.  No opposite charge: inf, -1.
  */
 __global__ void __launch_bounds__(256) partner_resolve_kernel(const float4* __restrict__ chg, const float4* __restrict__ blk,
-                                                              const float2* __restrict__ trk, long long first,
+                                                              const float2* __restrict__ trk, const int* __restrict__ perm,
+                                                              const int* __restrict__ inv, long long first,
                                                               long long count, long long n, float* __restrict__ out_d,
                                                               int* __restrict__ out_j)
 {
@@ -852,20 +882,22 @@ __global__ void __launch_bounds__(256) partner_resolve_kernel(const float4* __re
     if (w >= count) return;
     const long long i = first + w;
     const float4 t = chg[i];
+    const long long self = inv[i]; /* the blocks hold the charges in class order */
     const int b = __float_as_int(trk[w].y);
     double best = 1.0e300;
     int bj = 0x7fffffff;
     if (b >= 0) {
         const float4* src = blk + (long long)b * SBH + 1;
         for (int k = lane; k < SB; k += 32) {
-            const long long j = (long long)b * SB + k;
+            const long long js = (long long)b * SB + k;
             const float4 q = src[k];
-            if (j >= n || j == i || !(q.w * t.w < 0.f)) continue;
+            if (js >= n || js == self || !(q.w * t.w < 0.f)) continue;
             const double dx = (double)t.x - (double)q.x, dy = (double)t.y - (double)q.y, dz = (double)t.z - (double)q.z;
             const double d2 = dx * dx + dy * dy + dz * dz;
-            if (d2 < best) { /* ascending k per lane: the first (smallest) index wins ties */
+            const int j = perm[js]; /* the caller's index of that charge; the smallest one wins ties */
+            if (d2 < best || (d2 == best && j < bj)) {
                 best = d2;
-                bj = (int)j;
+                bj = j;
             }
         }
     }
@@ -894,85 +926,98 @@ __global__ void __launch_bounds__(256) partner_resolve_kernel(const float4* __re
  * measure-zero event for the path's inputs, so the list is almost always empty.  (The self term of a charge
  * is not such an event: it is excluded by index in self_block_loop.)
  */
+__device__ void repair_one(const EvalParams& P, const long long i, double (&red)[4][THREADS])
+{
+    const int tid = threadIdx.x;
+    const float4 t = P.tgt[i];
+    const double tx = t.x, ty = t.y, tz = t.z;
+    double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
+    /* the point source that IS target i (excluded by index, reading A3) */
+    const long long self = (P.self_first >= 0) ? (P.spos ? (long long)P.spos[i] : P.self_first + i) : -1;
+    for (int sct = 0; sct < 2; ++sct) {
+        const Section& S = P.sec[sct];
+        const double e2 = (double)S.eps2;
+        if (P.list != nullptr) {
+            if (sct != 0) continue;
+            /* LIST mode: the sources of target i are the blocks of its tile's list */
+            const long long tl = i / P.tt;
+            for (long long j = P.tile_ptr[tl] * SB + tid; j < P.tile_ptr[tl + 1] * SB; j += THREADS) {
+                const long long blk = P.list[j / SB];
+                const float4 q = P.pool[blk * SBH + 1 + (j % SB)];
+                if ((blk < P.list_self_blocks && blk * SB + (j % SB) == self) || q.w == 0.0f) continue;
+                const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
+                const double r2 = dx * dx + dy * dy + dz * dz + e2;
+                if (!(r2 > 0.0)) continue;
+                const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
+                ph += w;
+                ex += s3 * dx;
+                ey += s3 * dy;
+                ez += s3 * dz;
+            }
+        } else if (S.kind == KIND_POINTS) {
+            for (long long j = tid; j < S.nblk * SB; j += THREADS) {
+                const float4 q = S.src[(j / SB) * SBH + 1 + (j % SB)];
+                if ((sct == 0 && j == self) || q.w == 0.0f) continue;
+                const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
+                const double r2 = dx * dx + dy * dy + dz * dz + e2;
+                if (!(r2 > 0.0)) continue;
+                const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
+                ph += w;
+                ex += s3 * dx;
+                ey += s3 * dy;
+                ez += s3 * dz;
+            }
+        } else {
+            for (long long j = tid; j < S.npan * 7; j += THREADS) {
+                const long long pnl = j / 7;
+                const int k = (int)(j - pnl * 7);
+                const long long e = panel_entry(pnl);
+                const float4 o = S.src[e], q = S.qrel[j];
+                const float w = S.src[e + 2 + 2 * k].z;
+                if (w == 0.0f) continue;
+                /* shift into the frame in fp32 like the hot loop, then subtract the plain offset */
+                const double dx = (double)(t.x - o.x) - q.x, dy = (double)(t.y - o.y) - q.y,
+                             dz = (double)(t.z - o.z) - q.z;
+                const double r2 = dx * dx + dy * dy + dz * dz + e2;
+                if (!(r2 > 0.0)) continue;
+                const double u = rsqrt(r2), wu = (double)w * u, s3 = wu * u * u;
+                ph += wu;
+                ex += s3 * dx;
+                ey += s3 * dy;
+                ez += s3 * dz;
+            }
+        }
+    }
+    red[0][tid] = ex;
+    red[1][tid] = ey;
+    red[2][tid] = ez;
+    red[3][tid] = ph;
+    __syncthreads();
+    for (int h = THREADS / 2; h > 0; h >>= 1) {
+        if (tid < h)
+            for (int c = 0; c < 4; ++c) red[c][tid] += red[c][tid + h];
+        __syncthreads();
+    }
+    if (tid == 0)
+        P.out[i] = make_float4((float)(KE_D * red[0][0]), (float)(KE_D * red[1][0]), (float)(KE_D * red[2][0]),
+                               (float)(KE_D * red[3][0]));
+    __syncthreads();
+}
+
+/* P here is in the CALLER's target order: tgt[i] -> out[i], and target i is point source spos[i] (or self_first + i).
+ * The list holds output slots.  If more targets were reported than the list holds, every target whose result is not
+ * finite is recomputed instead (a guarded full pass over the results: nothing is silently left inf/NaN). */
 __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P)
 {
     __shared__ double red[4][THREADS];
-    const unsigned n = min(*P.bad_count, BAD_CAP);
-    const int tid = threadIdx.x;
-    for (unsigned r = blockIdx.x; r < n; r += gridDim.x) {
-        const long long i = P.bad_list[r];
-        const float4 t = P.tgt[i];
-        const double tx = t.x, ty = t.y, tz = t.z;
-        double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
-        for (int sct = 0; sct < 2; ++sct) {
-            const Section& S = P.sec[sct];
-            const double e2 = (double)S.eps2;
-            if (P.list != nullptr) {
-                if (sct != 0) continue;
-                /* LIST mode: the sources of target i are the blocks of its tile's list */
-                const long long tl = i / P.tt, self = P.self_first >= 0 ? P.self_first + i : -1;
-                for (long long j = P.tile_ptr[tl] * SB + tid; j < P.tile_ptr[tl + 1] * SB; j += THREADS) {
-                    const long long blk = P.list[j / SB];
-                    const float4 q = P.pool[blk * SBH + 1 + (j % SB)];
-                    if ((blk < P.list_self_blocks && blk * SB + (j % SB) == self) || q.w == 0.0f) continue;
-                    const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
-                    const double r2 = dx * dx + dy * dy + dz * dz + e2;
-                    if (!(r2 > 0.0)) continue;
-                    const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
-                    ph += w;
-                    ex += s3 * dx;
-                    ey += s3 * dy;
-                    ez += s3 * dz;
-                }
-            } else if (S.kind == KIND_POINTS) {
-                const long long self = (sct == 0 && P.self_first >= 0) ? P.self_first + i : -1;
-                for (long long j = tid; j < S.nblk * SB; j += THREADS) {
-                    const float4 q = S.src[(j / SB) * SBH + 1 + (j % SB)];
-                    if (j == self || q.w == 0.0f) continue;
-                    const double dx = tx - q.x, dy = ty - q.y, dz = tz - q.z;
-                    const double r2 = dx * dx + dy * dy + dz * dz + e2;
-                    if (!(r2 > 0.0)) continue;
-                    const double u = rsqrt(r2), w = (double)q.w * u, s3 = w * u * u;
-                    ph += w;
-                    ex += s3 * dx;
-                    ey += s3 * dy;
-                    ez += s3 * dz;
-                }
-            } else {
-                for (long long j = tid; j < S.npan * 7; j += THREADS) {
-                    const long long pnl = j / 7;
-                    const int k = (int)(j - pnl * 7);
-                    const long long e = panel_entry(pnl);
-                    const float4 o = S.src[e], q = S.qrel[j];
-                    const float w = S.src[e + 2 + 2 * k].z;
-                    if (w == 0.0f) continue;
-                    /* shift into the frame in fp32 like the hot loop, then subtract the plain offset */
-                    const double dx = (double)(t.x - o.x) - q.x, dy = (double)(t.y - o.y) - q.y,
-                                 dz = (double)(t.z - o.z) - q.z;
-                    const double r2 = dx * dx + dy * dy + dz * dz + e2;
-                    if (!(r2 > 0.0)) continue;
-                    const double u = rsqrt(r2), wu = (double)w * u, s3 = wu * u * u;
-                    ph += wu;
-                    ex += s3 * dx;
-                    ey += s3 * dy;
-                    ez += s3 * dz;
-                }
-            }
+    const unsigned n = *P.bad_count;
+    if (n <= BAD_CAP) {
+        for (unsigned r = blockIdx.x; r < n; r += gridDim.x) repair_one(P, P.bad_list[r], red);
+    } else {
+        for (long long i = blockIdx.x; i < P.nt; i += gridDim.x) {
+            const float4 o = P.out[i]; /* CTA-uniform */
+            if (!all_finite(o.x, o.y, o.z, o.w)) repair_one(P, i, red);
         }
-        red[0][tid] = ex;
-        red[1][tid] = ey;
-        red[2][tid] = ez;
-        red[3][tid] = ph;
-        __syncthreads();
-        for (int h = THREADS / 2; h > 0; h >>= 1) {
-            if (tid < h)
-                for (int c = 0; c < 4; ++c) red[c][tid] += red[c][tid + h];
-            __syncthreads();
-        }
-        if (tid == 0)
-            P.out[i] = make_float4((float)(KE_D * red[0][0]), (float)(KE_D * red[1][0]), (float)(KE_D * red[2][0]),
-                                   (float)(KE_D * red[3][0]));
-        __syncthreads();
     }
 }
 
@@ -982,19 +1027,61 @@ __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P
 constexpr float PAD_FAR = 1.0e15f;
 
 
-/* One CTA of SB threads per source block: plain copy (the targets of eval_at_charges), blocked copy with
- * header (the sources), padding (weight 0, parked far away so that it is never at zero distance from a
- * target), and the header's common weight (NaN if the block's weights differ). */
-__global__ void __launch_bounds__(SB) pack_charges_kernel(const float4* __restrict__ in, float4* __restrict__ plain,
-                                                           float4* __restrict__ blocked, long long n)
+/*
+ * Class order.  The fast loop (block_loop_uniform, 12 packed instructions) needs blocks whose 256 sources share one
+ * weight.  An avalanche creates electrons and ions in PAIRS, so the caller's array
+ * interleaves the signs; set_charges therefore sorts the sources, stably, by the ordered bit pattern of q (negative
+ * weights first, then -0, +0, positive): every block is uniform except the at most (classes - 1) blocks that straddle
+ * a class boundary, whatever order the caller uses.  The targets of an evaluation at the charges are taken in the
+ * same order (their own blocks stay contiguous: Eq 3.8's p != p' is an index test on ~TT/SB blocks per tile) and
+ * the results are scattered back to the caller's order when they are written.  An array that is already grouped by
+ * class in ascending q (electrons, then ions) keeps its order: the sort is stable.
+ */
+__device__ __forceinline__ unsigned weight_key(float q)
 {
-    const long long b = blockIdx.x, i = b * SB + threadIdx.x;
-    const float4 v = (i < n) ? in[i] : make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
-    if (i < n) plain[i] = v;
+    const unsigned u = __float_as_uint(q);
+    return u ^ ((u >> 31) ? 0xffffffffu : 0x80000000u); /* order-preserving: float order == unsigned order */
+}
+__global__ void __launch_bounds__(256) chg_key_kernel(const float4* __restrict__ in, unsigned* __restrict__ key,
+                                                     int* __restrict__ val, long long n)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    key[i] = weight_key(in[i].w);
+    val[i] = (int)i;
+}
+
+/* One CTA of SB threads per source block b of the class order (perm: class-order position -> input index): plain
+ * copy in input order, plain copy in class order (the targets of eval_at_charges), blocked copy with header (the
+ * sources), inverse permutation, padding (weight 0, parked far away so that it is never at zero distance from a
+ * target), and the header: .x = the weight all SB sources share (NaN if they differ), .y = their common sign +1, -1
+ * or 0 (NaN if the signs differ) -- padding counts as a member of either. */
+__global__ void __launch_bounds__(SB) pack_charges_kernel(const float4* __restrict__ in, const int* __restrict__ perm,
+                                                           float4* __restrict__ plain, float4* __restrict__ sorted,
+                                                           float4* __restrict__ blocked, int* __restrict__ inv,
+                                                           long long n)
+{
+    const long long b = blockIdx.x, s = b * SB + threadIdx.x;
+    float4 v = make_float4(PAD_FAR, PAD_FAR, PAD_FAR, 0.f);
+    if (s < n) {
+        plain[s] = in[s];
+        const int i = perm[s];
+        v = in[i];
+        sorted[s] = v;
+        inv[i] = (int)s;
+    }
     blocked[b * SBH + 1 + threadIdx.x] = v;
-    const float w0 = in[b * SB].w; /* b * SB < n for every launched block */
-    const int uniform = __syncthreads_and(v.w == w0);
-    if (threadIdx.x == 0) blocked[b * SBH] = make_float4(uniform ? w0 : __int_as_float(0x7fc00000), 0.f, 0.f, 0.f);
+    const float w0 = in[perm[b * SB]].w; /* b * SB < n for every launched block */
+    const float s0 = (w0 > 0.f) ? 1.f : ((w0 < 0.f) ? -1.f : 0.f);
+    const float sv = (v.w > 0.f) ? 1.f : ((v.w < 0.f) ? -1.f : 0.f);
+    const bool pad = !(s < n);
+    const int uniform = __syncthreads_and(pad || v.w == w0);
+    const int onesign = __syncthreads_and(pad || sv == s0);
+    const float nan = __int_as_float(0x7fc00000);
+    /* a short last block: its padding has weight 0, so a common weight w0 != 0 cannot be applied to the whole block */
+    const bool full = (b + 1) * SB <= n;
+    if (threadIdx.x == 0)
+        blocked[b * SBH] = make_float4((uniform && (full || w0 == 0.f)) ? w0 : nan, onesign ? s0 : nan, 0.f, 0.f);
 }
 
 /* 7-point degree-5 triangle rule (Radon): barycentric coordinate pattern (a, b, b) and weights,
@@ -1155,30 +1242,80 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) fma_probe_kernel(float* 
 
 namespace {
 
+/* selects the class-order positions s whose charge has an input index in [lo, hi) */
+struct InRange {
+    const int* perm;
+    int lo, hi;
+    __device__ __forceinline__ bool operator()(const int s) const
+    {
+        const int i = perm[s];
+        return i >= lo && i < hi;
+    }
+};
+
+/* the members of a sub-range in class order: coordinates and output slots from their positions */
+__global__ void __launch_bounds__(256) range_gather_kernel(const float4* __restrict__ sorted, const int* __restrict__ perm,
+                                                          const int* __restrict__ spos, float4* __restrict__ tgt,
+                                                          int* __restrict__ idx, int first, long long count)
+{
+    const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= count) return;
+    const int s = spos[j];
+    tgt[j] = sorted[s];
+    idx[j] = perm[s] - first;
+}
 
 long long pad_sb(long long n) { return ceil_div(n, SB) * SB; }
 long long pad_panels(long long np) { return ceil_div(np, PANELS_PER_BLOCK) * PANELS_PER_BLOCK; }
 
+template <class T>
+cudaError_t regrow(T*& p, size_t count)
+{
+    T* q = nullptr;
+    const cudaError_t e = cudaMalloc(&q, count * sizeof(T));
+    if (e != cudaSuccess) return e;
+    if (p) cudaFree(p);
+    p = q;
+    return cudaSuccess;
+}
+
+/* Library-owned charge buffers for n charges.  Growing them DISCARDS the current charge set (n_chg = -1: the next
+ * evaluation returns OBEM_ESTATE until obem_set_charges is called again) -- obem.h says so for obem_reserve. */
 int grow_charges(obem_ctx* c, long long n)
 {
     const long long need = pad_sb(n > 0 ? n : 1);
     if (need <= c->chg_cap) return OBEM_OK;
-    float4 *p = nullptr, *b = nullptr;
-    float2* t = nullptr;
-    OBEM_CUDA(c, cudaMalloc(&p, (size_t)need * sizeof(float4)));
-    cudaError_t e = cudaMalloc(&b, (size_t)(need / SB) * SBH * sizeof(float4));
-    if (e == cudaSuccess) e = cudaMalloc(&t, (size_t)need * sizeof(float2));
-    if (e != cudaSuccess) {
-        cudaFree(p);
-        if (b) cudaFree(b);
-        return cuda_fail(c, e);
+    c->n_chg = -1;
+    c->chg_cap = 0;
+    const size_t m = (size_t)need;
+    cudaError_t e = regrow(c->d_chg, m);
+    if (e == cudaSuccess) e = regrow(c->d_chg_blk, (size_t)(need / SB) * SBH);
+    if (e == cudaSuccess) e = regrow(c->d_trk, m);
+    if (e == cudaSuccess) e = regrow(c->d_chg_sorted, m);
+    if (e == cudaSuccess) e = regrow(c->d_perm, m);
+    if (e == cudaSuccess) e = regrow(c->d_inv, m);
+    if (e == cudaSuccess) e = regrow(c->d_skey[0], m);
+    if (e == cudaSuccess) e = regrow(c->d_skey[1], m);
+    if (e == cudaSuccess) e = regrow(c->d_sval, m);
+    if (e == cudaSuccess) e = regrow(c->d_rng_spos, m);
+    if (e == cudaSuccess) e = regrow(c->d_rng_idx, m);
+    if (e == cudaSuccess) e = regrow(c->d_rng_tgt, m);
+    if (e == cudaSuccess && !c->d_rng_num) e = regrow(c->d_rng_num, 64);
+    if (e == cudaSuccess) { /* CUB workspace: the larger of the radix sort's and the select's */
+        size_t b_sort = 0, b_sel = 0;
+        e = cub::DeviceRadixSort::SortPairs(nullptr, b_sort, c->d_skey[0], c->d_skey[1], c->d_sval, c->d_perm, (int)need);
+        if (e == cudaSuccess)
+            e = cub::DeviceSelect::If(nullptr, b_sel, thrust::counting_iterator<int>(0), c->d_rng_spos, c->d_rng_num,
+                                      (int)need, InRange{c->d_perm, 0, 0});
+        const size_t want = (b_sort > b_sel ? b_sort : b_sel) + 256;
+        if (e == cudaSuccess && want > c->sort_tmp_cap) {
+            char* t = (char*)c->d_sort_tmp;
+            e = regrow(t, want);
+            c->d_sort_tmp = t;
+            if (e == cudaSuccess) c->sort_tmp_cap = want;
+        }
     }
-    if (c->d_chg) cudaFree(c->d_chg);
-    if (c->d_chg_blk) cudaFree(c->d_chg_blk);
-    if (c->d_trk) cudaFree(c->d_trk);
-    c->d_chg = p;
-    c->d_chg_blk = b;
-    c->d_trk = t;
+    if (e != cudaSuccess) return cuda_fail(c, e);
     c->chg_cap = need;
     return OBEM_OK;
 }
@@ -1187,6 +1324,8 @@ int grow_panels(obem_ctx* c, long long np)
 {
     const long long need = np > 0 ? np : 1;
     if (need <= c->pan_cap) return OBEM_OK;
+    c->n_pan = -1; /* growing DISCARDS the current panel set (see grow_charges) */
+    c->near_valid = 0;
     float4 *p = nullptr, *qp = nullptr, *nr = nullptr, *it = nullptr, *qr = nullptr;
     double* a = nullptr;
     cudaError_t e = cudaMalloc(&p, (size_t)(pad_panels(need) / PPB) * SBH_P * sizeof(float4));
@@ -1238,8 +1377,10 @@ int grow_stage(obem_ctx* c, int i, size_t bytes)
 int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                        float eps_nbody, cudaStream_t st, float2* trk_out)
 {
-    if (flags & ~(OBEM_NBODY | OBEM_PANELS | OBEM_PANELS_EXACT)) return OBEM_EINVAL;
+    if (flags & ~(OBEM_NBODY | OBEM_PANELS | OBEM_PANELS_EXACT | OBEM_NO_PHI)) return OBEM_EINVAL;
     if ((flags & OBEM_PANELS_EXACT) && !(flags & OBEM_PANELS)) return OBEM_EINVAL;
+    /* E only: not with the exact near-field correction or the partner by-product (their kernels carry phi) */
+    if ((flags & OBEM_NO_PHI) && ((flags & OBEM_PANELS_EXACT) || trk_out)) return OBEM_EINVAL;
     if ((flags & OBEM_NBODY) && c->n_chg < 0) return OBEM_ESTATE;
     if ((flags & OBEM_PANELS) && c->n_pan < 0) return OBEM_ESTATE;
     if (nt == 0) return OBEM_OK;
@@ -1248,7 +1389,8 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     /* NEXT-3: exact integrals for the panels near each target (obem_near.cu) */
     if ((flags & OBEM_PANELS_EXACT) && c->n_pan > 0)
         return obem_eval_exact(c, tgt, nt, out, flags & ~OBEM_PANELS_EXACT, self_first, eps_nbody, st, trk_out);
-    flags &= ~OBEM_PANELS_EXACT;
+    const bool phi = !(flags & OBEM_NO_PHI);
+    flags &= ~(OBEM_PANELS_EXACT | OBEM_NO_PHI);
 
     EvalParams P;
     int ns = 0;
@@ -1303,6 +1445,8 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
     P.accumulate = 0;
     P.trk_out = trk_out;
     P.trk_ws = c->d_trk_ws;
+    P.out_idx = nullptr;
+    P.spos = nullptr;
     OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
 
     /* one stream-K launch (+ fix-up) per section; the second adds to the first's result */
@@ -1317,22 +1461,53 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
             Q.tt = PANEL_TT;
             Q.ws_stride = TT_MAX;
             Q.ntiles = ceil_div(nt, (long long)PANEL_TT);
+        } else if (P.self_first >= 0) {
+            /* Evaluation at the charges [self_first, self_first + nt): the N-body launch takes its targets in CLASS
+             * ORDER (pack_charges_kernel says why) and scatters the results to the caller's order. */
+            if (P.self_first == 0 && nt == c->n_chg) {
+                Q.tgt = c->d_chg_sorted; /* target i is source i */
+                Q.out_idx = c->d_perm;
+            } else {
+                /* a sub-range: its members in class order (stable select over the class-order positions), with
+                 * their positions -- the kernel finds each tile's own blocks from them */
+                size_t tmp = c->sort_tmp_cap;
+                OBEM_CUDA(c, cub::DeviceSelect::If(c->d_sort_tmp, tmp, thrust::counting_iterator<int>(0), c->d_rng_spos,
+                                                   c->d_rng_num, (int)c->n_chg,
+                                                   InRange{c->d_perm, (int)P.self_first, (int)(P.self_first + nt)}, st));
+                range_gather_kernel<<<(unsigned)ceil_div(nt, 256), 256, 0, st>>>(
+                    c->d_chg_sorted, c->d_perm, c->d_rng_spos, c->d_rng_tgt, c->d_rng_idx, (int)P.self_first, nt);
+                OBEM_CUDA(c, cudaGetLastError());
+                c->launches += 2;
+                Q.tgt = c->d_rng_tgt;
+                Q.out_idx = c->d_rng_idx;
+                Q.spos = c->d_rng_spos;
+                Q.self_first = 0;
+            }
         }
         Q.U = Q.ntiles * Q.nblk;
         Q.accumulate = (k > 0);
         if (Q.sec[0].kind == KIND_PANELS) {
             Q.self_first = -1;
             Q.trk_out = nullptr;
-            obem_panels_kernel<PANEL_NPAIR><<<c->grid, THREADS, 0, st>>>(Q);
+            if (phi) obem_panels_kernel<PANEL_NPAIR, true><<<c->grid, THREADS, ACC_BYTES_PANELS, st>>>(Q);
+            else obem_panels_kernel<PANEL_NPAIR, false><<<c->grid, THREADS, ACC_BYTES_PANELS, st>>>(Q);
         } else if (Q.trk_out) {
-            obem_eval_kernel<KIND_POINTS, true><<<c->grid, THREADS, 0, st>>>(Q);
+            obem_eval_kernel<true, false, true><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
+        } else if (phi) {
+            obem_eval_kernel<false, false, true><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
         } else {
-            obem_eval_kernel<KIND_POINTS, false><<<c->grid, THREADS, 0, st>>>(Q);
+            obem_eval_kernel<false, false, false><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
         }
         OBEM_CUDA(c, cudaGetLastError());
-        obem_fixup_kernel<<<(unsigned)Q.ntiles, THREADS, 0, st>>>(Q, c->grid);
+        obem_fixup_kernel<<<dim3((unsigned)Q.ntiles, (unsigned)Q.tpt), THREADS, (size_t)(c->grid + 2) * sizeof(long long),
+                            st>>>(Q, c->grid);
         OBEM_CUDA(c, cudaGetLastError());
         c->launches += 2;
+    }
+    /* the repair pass works in the caller's order: target i of `tgt` is point source inv[self_first + i] */
+    if (P.self_first >= 0 && (flags & OBEM_NBODY) && c->n_chg > 0) {
+        P.spos = c->d_inv + P.self_first;
+        P.self_first = 0;
     }
     obem_repair_kernel<<<c->sm_count, THREADS, 0, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
@@ -1373,6 +1548,8 @@ int obem_eval_list(obem_ctx* c, const float4* tgt, long long nt, float4* out, co
     P.trk_out = nullptr;
     P.trk_ws = c->d_trk_ws;
     P.accumulate = 0;
+    P.out_idx = nullptr;
+    P.spos = nullptr;
     P.tile_ptr = tile_ptr;
     P.list = list;
     P.pool = pool;
@@ -1381,9 +1558,10 @@ int obem_eval_list(obem_ctx* c, const float4* tgt, long long nt, float4* out, co
     P.bad_count = c->d_bad_count;
     P.bad_list = c->d_bad_list;
     OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
-    obem_eval_kernel<KIND_POINTS, false, true><<<c->grid, THREADS, 0, st>>>(P);
+    obem_eval_kernel<false, true, true><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
-    obem_fixup_kernel<<<(unsigned)P.ntiles, THREADS, 0, st>>>(P, c->grid);
+    obem_fixup_kernel<<<dim3((unsigned)P.ntiles, (unsigned)P.tpt), THREADS, (size_t)(c->grid + 2) * sizeof(long long), st>>>(
+        P, c->grid);
     OBEM_CUDA(c, cudaGetLastError());
     obem_repair_kernel<<<c->sm_count, THREADS, 0, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
@@ -1431,7 +1609,15 @@ int obem_create(obem_ctx** out, int device)
     }
     c->sm_count = prop.multiProcessorCount;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<KIND_POINTS, true>, THREADS, 0);
+    /* the running sums of the evaluation kernels live in dynamic shared memory beyond the 48 KB default */
+    e = cudaFuncSetAttribute(obem_eval_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_panels_kernel<PANEL_NPAIR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_PANELS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_panels_kernel<PANEL_NPAIR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_PANELS);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<true, false, true>, THREADS, ACC_BYTES_POINTS);
     if (e != cudaSuccess || per_sm < 1) {
         /* no sm_100a code for this device, or the kernel cannot be resident */
         cudaGetLastError();
@@ -1440,7 +1626,7 @@ int obem_create(obem_ctx** out, int device)
     }
     if (per_sm > CTAS_PER_SM) per_sm = CTAS_PER_SM;
     c->grid = c->sm_count * per_sm;
-    e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT_MAX * sizeof(float4));
+    e = cudaMalloc(&c->d_ws, (size_t)c->grid * 2 * TT_MAX * 4 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_trk_ws, (size_t)c->grid * 2 * TT_MAX * sizeof(float2));
     if (e == cudaSuccess) e = cudaMalloc(&c->d_sink, 256);
     if (e == cudaSuccess) e = cudaMalloc(&c->d_bad_count, 256);
@@ -1462,6 +1648,17 @@ int obem_destroy(obem_ctx* c)
     cudaDeviceSynchronize();
     if (c->d_chg) cudaFree(c->d_chg);
     if (c->d_chg_blk) cudaFree(c->d_chg_blk);
+    if (c->d_chg_sorted) cudaFree(c->d_chg_sorted);
+    if (c->d_perm) cudaFree(c->d_perm);
+    if (c->d_inv) cudaFree(c->d_inv);
+    if (c->d_skey[0]) cudaFree(c->d_skey[0]);
+    if (c->d_skey[1]) cudaFree(c->d_skey[1]);
+    if (c->d_sval) cudaFree(c->d_sval);
+    if (c->d_sort_tmp) cudaFree(c->d_sort_tmp);
+    if (c->d_rng_spos) cudaFree(c->d_rng_spos);
+    if (c->d_rng_idx) cudaFree(c->d_rng_idx);
+    if (c->d_rng_tgt) cudaFree(c->d_rng_tgt);
+    if (c->d_rng_num) cudaFree(c->d_rng_num);
     if (c->d_psrc) cudaFree(c->d_psrc);
     if (c->d_area) cudaFree(c->d_area);
     if (c->d_qpts) cudaFree(c->d_qpts);
@@ -1542,16 +1739,23 @@ int obem_set_sigma(obem_ctx* c, const float* d_sigma, int64_t n_panels, void* cu
 
 int obem_set_charges(obem_ctx* c, const float* d_xyzq, int64_t n, void* cuda_stream)
 {
-    if (!c || n < 0) return OBEM_EINVAL;
+    if (!c || n < 0 || n > 0x7fffff00LL) return OBEM_EINVAL; /* class-order positions are 32-bit */
     if (n > 0 && (!d_xyzq || !aligned16(d_xyzq))) return OBEM_EINVAL;
     DeviceGuard g(c->device);
     int rc = grow_charges(c, n);
     if (rc != OBEM_OK) return rc;
     if (n > 0) {
-        pack_charges_kernel<<<(unsigned)ceil_div(n, SB), SB, 0, (cudaStream_t)cuda_stream>>>(
-            (const float4*)d_xyzq, c->d_chg, c->d_chg_blk, n);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        /* class order: stable radix sort of (ordered bits of q, index), then one gather pass */
+        chg_key_kernel<<<(unsigned)ceil_div(n, 256), 256, 0, st>>>((const float4*)d_xyzq, c->d_skey[0], c->d_sval, n);
         OBEM_CUDA(c, cudaGetLastError());
-        c->launches += 1;
+        size_t tmp = c->sort_tmp_cap;
+        OBEM_CUDA(c, cub::DeviceRadixSort::SortPairs(c->d_sort_tmp, tmp, c->d_skey[0], c->d_skey[1], c->d_sval, c->d_perm,
+                                                     (int)n, 0, 32, st));
+        pack_charges_kernel<<<(unsigned)ceil_div(n, SB), SB, 0, st>>>((const float4*)d_xyzq, c->d_perm, c->d_chg,
+                                                                     c->d_chg_sorted, c->d_chg_blk, c->d_inv, n);
+        OBEM_CUDA(c, cudaGetLastError());
+        c->launches += 3; /* + the radix sort's own passes */
     }
     c->n_chg = n;
     return OBEM_OK;
@@ -1590,8 +1794,9 @@ int obem_eval_at_charges_partners_range(obem_ctx* c, int64_t first, int64_t coun
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int rc = obem_eval_internal(c, c->d_chg + first, count, (float4*)d_out, flags, first, c->eps_pp, st, c->d_trk);
     if (rc != OBEM_OK) return rc;
-    partner_resolve_kernel<<<(unsigned)ceil_div(count, 8), 256, 0, st>>>(c->d_chg, c->d_chg_blk, c->d_trk, first, count,
-                                                                       c->n_chg, d_partner_d, d_partner_j);
+    partner_resolve_kernel<<<(unsigned)ceil_div(count, 8), 256, 0, st>>>(c->d_chg, c->d_chg_blk, c->d_trk, c->d_perm,
+                                                                       c->d_inv, first, count, c->n_chg, d_partner_d,
+                                                                       d_partner_j);
     OBEM_CUDA(c, cudaGetLastError());
     c->launches += 1;
     return OBEM_OK;

@@ -145,9 +145,23 @@ struct obem_ctx {
     float eps_pp = 0.f, eps_panel = 0.f;
     /* charges */
     float4* d_chg = nullptr;     /* plain copy [n]: the targets of eval_at_charges                */
-    float4* d_chg_blk = nullptr; /* blocked copy with headers [nblk][SBH]: the sources            */
+    float4* d_chg_blk = nullptr; /* blocked copy with headers [nblk][SBH]: the sources, in CLASS ORDER */
     long long chg_cap = 0;       /* capacity in charges (a multiple of SB)                        */
     long long n_chg = -1;
+    /* class order: the charges stably sorted by q (set_charges), so that the 256-source blocks are weight-uniform
+     * whatever order the caller stores electrons and ions in */
+    float4* d_chg_sorted = nullptr; /* [chg_cap] plain copy in class order: the targets of eval_at_charges          */
+    int* d_perm = nullptr;          /* [chg_cap] class-order position -> input index                                */
+    int* d_inv = nullptr;           /* [chg_cap] input index -> class-order position                                */
+    unsigned* d_skey[2] = {nullptr, nullptr}; /* [chg_cap] sort keys (ordered bit pattern of q), in / out           */
+    int* d_sval = nullptr;          /* [chg_cap] 0, 1, 2, ...: the values the sort permutes                         */
+    void* d_sort_tmp = nullptr;     /* CUB workspace (radix sort, select)                                           */
+    size_t sort_tmp_cap = 0;
+    /* evaluation at a sub-range [first, first + count) of the charges: its members in class order */
+    int* d_rng_spos = nullptr;      /* [chg_cap] their class-order positions, ascending                             */
+    int* d_rng_idx = nullptr;       /* [chg_cap] their output slots (input index - first)                           */
+    float4* d_rng_tgt = nullptr;    /* [chg_cap] their coordinates                                                  */
+    int* d_rng_num = nullptr;       /* [1] how many the select wrote (== count)                                     */
     /* panels */
     float4* d_psrc = nullptr;
     double* d_area = nullptr;
@@ -160,7 +174,7 @@ struct obem_ctx {
     /* split-tile workspace [grid][2][TT] */
     float2* d_trk = nullptr;     /* [chg_cap] (min softened r2 to an opposite charge, its source block) per charge */
     float2* d_trk_ws = nullptr;  /* [grid][2][TT] the same for split tiles                                        */
-    float4* d_ws = nullptr;
+    double* d_ws = nullptr;      /* [grid][2][TT_MAX][4] fp64 partial sums of split tiles */
     float* d_sink = nullptr;
     unsigned* d_bad_count = nullptr;
     long long* d_bad_list = nullptr;

@@ -259,7 +259,8 @@ int field_at_state(obem_ctx* c, const float* d_xyzq, long long n, unsigned flags
 {
     int rc = obem_set_charges(c, d_xyzq, n, stream);
     if (rc != OBEM_OK) return rc;
-    return obem_eval_at_charges(c, (float*)c->d_step_field, flags, stream);
+    /* the kicks read only E: the E-only instantiations of the evaluation kernels */
+    return obem_eval_at_charges(c, (float*)c->d_step_field, flags | OBEM_NO_PHI, stream);
 }
 
 int step_args_ok(obem_ctx* c, const float* d_xyzq, const float* d_vel, int64_t n, unsigned flags)

@@ -341,6 +341,20 @@ def make_workload(cfg: int, charge_div: int = 1, mesh_div: int = 1, point_div: i
                     sigma.astype(np.float32), 0.0, points=pts.reshape(-1, 4), meta=meta)
 
 
+def pair_creation_order(wl: Workload, seed: int = 0) -> Workload:
+    """The same charges in the order an avalanche stores them.  The generators above write all electrons, then all
+    ions; the method creates electrons and ions in PAIRS as the avalanche grows, so its
+    particle array interleaves the signs.  Stand-in: a seeded random permutation of the config's charges
+    (`meta["perm"]`: position in the returned array -> position in `wl`); panels and points are unchanged."""
+    if wl.n_charges == 0:
+        return wl
+    perm = np.random.default_rng([1, wl.cfg, seed]).permutation(wl.n_charges)
+    meta = dict(wl.meta)
+    meta["perm"] = perm
+    return Workload(wl.name + "-pair-order", wl.cfg, np.ascontiguousarray(wl.xyzq[perm]), wl.verts, wl.sigma, wl.eps_pp,
+                    wl.eps_panel, wl.points, meta)
+
+
 def random_rotation(rng):
     """A proper 3x3 rotation matrix (QR of a Gaussian matrix), for invariance tests."""
     a = rng.normal(size=(3, 3))
