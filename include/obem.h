@@ -193,6 +193,22 @@ int obem_apply_inverse(obem_ctx* c, const float* d_minv, int64_t n, int64_t ld, 
 int obem_update_sigma_dynamic(obem_ctx* c, const int32_t* d_kind, const float* d_bc, const float* d_deps,
                               const float* d_minv, int64_t ld, float* d_sigma, void* cuda_stream);
 
+/* Several charge-density vectors on the SAME cells in one pass.  The signal induced on a read-out electrode is
+ * computed with the Shockley-Ramo theorem from that electrode's weighting field (section 3.3.4,
+ * Eq 3.13): the field of the set-up with that electrode at unit potential and the others grounded -- one more
+ * solution sigma^(e) of the same BEM matrix, evaluated with the same Eq (2.13)/(2.14) at the same
+ * points.  The distance / rsqrt work of every (quadrature point, target) pair does not depend on sigma and is shared:
+ *   d_sigma [n_sigma][n_panels] fp32 [C/m^2] (row s = density vector s; the sigma given to obem_set_panels /
+ *           obem_set_sigma is NOT used and not changed)
+ *   d_pts   [m][4] fp32, 4th lane ignored;   d_out [n_sigma][m][4] fp32 = Ex, Ey, Ez [V/m], phi [V] of vector s.
+ * Up to 4 vectors per pass over the geometry (103 packed FP32 instructions per panel and target pair for 4 vectors
+ * against 4 x 87 for four obem_set_sigma + obem_eval_at_points rounds); more vectors take ceil(n_sigma / 4)
+ * passes.  eps_panel and reading A4 (zero distance contributes 0) apply as in obem_eval_at_points.  Library-owned
+ * buffers (the unit-density encoding of the geometry, built on the first call after obem_set_panels; one pass's
+ * blocked sigma rows) grow with cudaMalloc on the first call of a given size.  OBEM_ESTATE before obem_set_panels. */
+int obem_eval_panels_multi(obem_ctx* c, const float* d_sigma, int n_sigma, const float* d_pts, int64_t m,
+                           float* d_out, void* cuda_stream);
+
 /* ----------------------------------------------------------------------------------------------------------
  * NEXT-2: numerical integrators, section 3.2.5 -- the consumers of the field evaluation.
  * State: d_xyzq [n][4] fp32 = x, y, z [m], q [C];  d_vel [n][4] fp32 = vx, vy, vz [m/s], m [kg] (m = 0: immobile).

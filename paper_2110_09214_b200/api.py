@@ -55,6 +55,7 @@ SIGNATURES = {
     "obem_update_sigma_dynamic": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, _c_fp, _i64, _c_fp,
                                                  ctypes.c_void_p]),
     "obem_get_panel_normals": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
+    "obem_eval_panels_multi": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_int, _c_fp, _i64, _c_fp, ctypes.c_void_p]),
     # NEXT-2: recombination by-product of the N-body pass
     "obem_eval_at_charges_partners": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, ctypes.c_uint,
                                                      ctypes.c_void_p]),
@@ -398,6 +399,30 @@ class Context:
                                                    sigma.data_ptr() if n else None, _stream_ptr(stream)),
                     "obem_update_sigma_dynamic")
         return sigma
+
+    def eval_panels_multi(self, sigmas, pts, out=None, stream=None):
+        """Eq (2.13)/(2.14) for several density vectors on the current cells (weighting fields, Eq 3.13):
+        sigmas [K, Np], pts [M, 4] -> out [K, M, 4]."""
+        torch = _torch()
+        k, m = int(sigmas.shape[0]), int(pts.shape[0])
+        npan = max(self.n_panels, 0)
+        if k and npan:
+            _dev_f32(sigmas, "sigmas")
+            if sigmas.dim() != 2 or sigmas.shape[1] != npan:
+                raise ValueError("sigmas must be [K, n_panels]")
+        if m:
+            _dev_f32(pts, "pts", (4,))
+        if out is None:
+            out = torch.empty((k, m, 4), dtype=torch.float32, device="cuda:%d" % self.device)
+        elif k and m:
+            _dev_f32(out, "out", (4,))
+            if tuple(out.shape) != (k, m, 4):
+                raise ValueError("out must be [K, M, 4]")
+        self._check(_lib.obem_eval_panels_multi(self._h, sigmas.data_ptr() if (k and npan) else None, k,
+                                                pts.data_ptr() if m else None, m,
+                                                out.data_ptr() if (k and m) else None, _stream_ptr(stream)),
+                    "obem_eval_panels_multi")
+        return out
 
     def get_panel_normals(self, stream=None):
         n = max(self.n_panels, 0)

@@ -58,11 +58,7 @@ constexpr int TT = THREADS * TPT;     /* targets per tile                       
 #ifndef OBEM_PANEL_TPT
 #define OBEM_PANEL_TPT 10
 #endif
-#ifndef OBEM_PANEL_DEPTH
-#define OBEM_PANEL_DEPTH 5
-#endif
 constexpr int PANEL_NPAIR = OBEM_PANEL_TPT / 2;
-constexpr int PANEL_DEPTH = OBEM_PANEL_DEPTH;
 constexpr int PANEL_TT = THREADS * OBEM_PANEL_TPT;
 constexpr int TT_MAX = PANEL_TT > TT ? PANEL_TT : TT; /* workspace slots are sized for the larger tile */
 static_assert(OBEM_PANEL_TPT % 2 == 0, "bad tuning knobs");
@@ -101,11 +97,6 @@ constexpr int KIND_POINTS = 0, KIND_PANELS = 1;
  * not (then .y.. unused).  Identical particles (electrons, singly charged ions) make whole blocks uniform,
  * and a uniform block needs one packed instruction less per interaction (block_loop_uniform). */
 constexpr int SBH = SB + 1;
-/* Panel blocks: PPB panels x (1 origin + 7 x 2) float4 = 510 of 512 slots, + header. */
-constexpr int PPB = 34;
-constexpr int PANEL_SLOTS = 15;
-constexpr int SBH_P = 512 + 1;
-constexpr int PANELS_PER_BLOCK = PPB;
 
 struct EvalParams {
     Section sec[2];
@@ -140,7 +131,7 @@ struct EvalParams {
     const int* spos;      /* != NULL: target i IS point source spos[i] of sec[0] (ascending in i);
                              NULL: it is source self_first + i                                                   */
 };
-constexpr unsigned BAD_CAP = 1u << 20;
+constexpr unsigned BAD_CAP = 1u << 16;
 /* dynamic shared memory of the evaluation kernels: their fp64 running sums (acc_flush) */
 constexpr size_t ACC_BYTES_POINTS = (size_t)8 * NPAIR * THREADS * sizeof(double);
 constexpr size_t ACC_BYTES_PANELS = (size_t)8 * PANEL_NPAIR * THREADS * sizeof(double);
@@ -258,6 +249,53 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
     }
 }
 
+/* Statement-order knobs of the uniform loop.  ptxas schedules the ~235-instruction trip itself, and on two warps per
+ * SM sub-partition the result decides +-3 % of the launch (measured: 420 .. 447 ms on config 3 over 36 orders that
+ * differ in nothing else), so the order is a tuned parameter per instantiation -- VE: order of the three E FMAs,
+ * VP: where the phi add sits, D: pipeline distance, VF: order of the r2 FMAs.  DESIGN.md section 5 has the sweep. */
+/* each knob set is four decimal digits: D, VE, VP, VF */
+#ifndef OBEM_KNOBS_PHI
+#define OBEM_KNOBS_PHI 4220
+#endif
+#ifndef OBEM_KNOBS_E
+#define OBEM_KNOBS_E 5300
+#endif
+#ifndef OBEM_KNOBS_T
+#define OBEM_KNOBS_T 3000
+#endif
+/* the same for the panel loop (VF unused) */
+#ifndef OBEM_PKNOBS_PHI
+#define OBEM_PKNOBS_PHI 5200
+#endif
+#ifndef OBEM_PKNOBS_E
+#define OBEM_PKNOBS_E 5200
+#endif
+struct Knobs {
+    int d, ve, vp, vf;
+};
+constexpr Knobs knobs_of(int code) { return Knobs{code / 1000, (code / 100) % 10, (code / 10) % 10, code % 10}; }
+constexpr Knobs KNOBS_PHI = knobs_of(OBEM_KNOBS_PHI), KNOBS_E = knobs_of(OBEM_KNOBS_E), KNOBS_T = knobs_of(OBEM_KNOBS_T);
+constexpr Knobs PKNOBS_PHI = knobs_of(OBEM_PKNOBS_PHI), PKNOBS_E = knobs_of(OBEM_PKNOBS_E);
+
+template <int VF>
+__device__ __forceinline__ void uni_front(u64& dx, u64& dy, u64& dz, u64& u, float& r2l, float& r2h, const u64 tx,
+                                          const u64 ty, const u64 tz, const float sx, const float sy, const float sz,
+                                          const u64 e2)
+{
+    dx = sub2(tx, pk(sx, sx));
+    dy = sub2(ty, pk(sy, sy));
+    dz = sub2(tz, pk(sz, sz));
+    u64 r2;
+    if (VF == 0) { r2 = fma2(dx, dx, e2); r2 = fma2(dy, dy, r2); r2 = fma2(dz, dz, r2); }
+    if (VF == 1) { r2 = fma2(dz, dz, e2); r2 = fma2(dy, dy, r2); r2 = fma2(dx, dx, r2); }
+    if (VF == 2) { r2 = fma2(dy, dy, e2); r2 = fma2(dx, dx, r2); r2 = fma2(dz, dz, r2); }
+    if (VF == 3) { r2 = fma2(dx, dx, e2); r2 = fma2(dz, dz, r2); r2 = fma2(dy, dy, r2); }
+    if (VF == 4) { r2 = fma2(dy, dy, e2); r2 = fma2(dz, dz, r2); r2 = fma2(dx, dx, r2); }
+    if (VF == 5) { r2 = fma2(dz, dz, e2); r2 = fma2(dx, dx, r2); r2 = fma2(dy, dy, r2); }
+    upk(r2, r2l, r2h);
+    u = pk(rsqrt_approx(r2l), rsqrt_approx(r2h));
+}
+
 /*
  * Same for a block whose SB sources all carry the weight w (header): sum_j w f(r_j) = w sum_j f(r_j), so the
  * weight is applied once per block and the body is 12 packed instructions: phi += u, u^2, u^3, E += u^3 d.
@@ -268,6 +306,8 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
                                                    u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
 {
+    constexpr Knobs KN = TRACK ? KNOBS_T : (PHI ? KNOBS_PHI : KNOBS_E);
+    constexpr int DEPTH = KN.d;
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR;
 #pragma unroll 1
@@ -280,26 +320,26 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
+                float r2l, r2h;
+                uni_front<KN.vf>(dX[k], dY[k], dZ[k], U[k], r2l, r2h, X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
                 if (TRACK) {
-                    /* by-product: smallest softened r2 of the block per target, 2 FMNMX on the
+                    /* by-product: smallest softened r2 of the block per target, 2 VIMNMX on the
                      * otherwise idle ALU pipe; whether the block's sign is opposite is decided after the block */
-                    float r2l, r2h;
-                    item_front_r2<false>(dX[k], dY[k], dZ[k], U[k], r2l, r2h, X[p], Y[p], Z[p], q[j].x, q[j].y,
-                                         q[j].z, e2);
                     bm[2 * p] = min_nonneg(bm[2 * p], r2l);
                     bm[2 * p + 1] = min_nonneg(bm[2 * p + 1], r2h);
-                } else {
-                    item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
                 }
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, p = kk % NPAIR;
-                if (PHI) aP[p] = add2(aP[p], U[kk]);
+                if (PHI && KN.vp == 0) aP[p] = add2(aP[p], U[kk]);
                 const u64 u2 = mul2(U[kk], U[kk]);
                 const u64 u3 = mul2(u2, U[kk]);
-                aX[p] = fma2(u3, dX[kk], aX[p]);
-                aY[p] = fma2(u3, dY[kk], aY[p]);
-                aZ[p] = fma2(u3, dZ[kk], aZ[p]);
+                if (PHI && KN.vp == 1) aP[p] = add2(aP[p], U[kk]);
+                if (KN.ve == 0) { aX[p] = fma2(u3, dX[kk], aX[p]); aY[p] = fma2(u3, dY[kk], aY[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); }
+                if (KN.ve == 1) { aZ[p] = fma2(u3, dZ[kk], aZ[p]); aY[p] = fma2(u3, dY[kk], aY[p]); aX[p] = fma2(u3, dX[kk], aX[p]); }
+                if (KN.ve == 2) { aY[p] = fma2(u3, dY[kk], aY[p]); aX[p] = fma2(u3, dX[kk], aX[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); }
+                if (KN.ve == 3) { aX[p] = fma2(u3, dX[kk], aX[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); aY[p] = fma2(u3, dY[kk], aY[p]); }
+                if (PHI && KN.vp == 2) aP[p] = add2(aP[p], U[kk]);
             }
         }
     }
@@ -334,8 +374,9 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
                                            const u64 (&Y)[NP], const u64 (&Z)[NP], u64 (&aX)[NP],
                                            u64 (&aY)[NP], u64 (&aZ)[NP], u64 (&aP)[NP])
 {
-    constexpr int NPAIR = NP;          /* shadows the point kernel's pair count */
-    constexpr int DEPTH = PANEL_DEPTH; /* and its pipeline distance */
+    constexpr int NPAIR = NP; /* shadows the point kernel's pair count */
+    constexpr Knobs KN = PHI ? PKNOBS_PHI : PKNOBS_E;
+    constexpr int DEPTH = KN.d; /* and its pipeline distance */
     constexpr int K = 7 * NPAIR;
 #pragma unroll 1
     for (int pp = 0; pp < PPB; ++pp) {
@@ -379,12 +420,15 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
-                if (PHI) aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
+                if (PHI && KN.vp == 0) aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
                 const u64 u2 = mul2(U[kk], U[kk]);
                 const u64 u3 = mul2(u2, U[kk]);
-                aX[p] = fma2(u3, dX[kk], aX[p]);
-                aY[p] = fma2(u3, dY[kk], aY[p]);
-                aZ[p] = fma2(u3, dZ[kk], aZ[p]);
+                if (PHI && KN.vp == 1) aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
+                if (KN.ve == 0) { aX[p] = fma2(u3, dX[kk], aX[p]); aY[p] = fma2(u3, dY[kk], aY[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); }
+                if (KN.ve == 1) { aZ[p] = fma2(u3, dZ[kk], aZ[p]); aY[p] = fma2(u3, dY[kk], aY[p]); aX[p] = fma2(u3, dX[kk], aX[p]); }
+                if (KN.ve == 2) { aY[p] = fma2(u3, dY[kk], aY[p]); aX[p] = fma2(u3, dX[kk], aX[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); }
+                if (KN.ve == 3) { aX[p] = fma2(u3, dX[kk], aX[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); aY[p] = fma2(u3, dY[kk], aY[p]); }
+                if (PHI && KN.vp == 2) aP[p] = fma2(U[kk], pk(qb[j].x, qb[j].x), aP[p]);
             }
         }
     }
@@ -603,11 +647,11 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
         /* blocks of sec[0] that hold this tile's own targets (evaluation at the charges): the targets are in the
          * sources' order, so these are the blocks [dlo, dhi] of its first and last target -- exactly (spos == NULL:
          * the whole set) or as a hull that is refined per block (a sub-range straddles the class boundaries) */
-        long long dlo = 0, dhi = -1;
+        int dlo = 0, dhi = -1;
         if (P.self_first >= 0) {
             const long long t0 = tile * (long long)TT, t1 = min(t0 + TT, P.nt) - 1;
-            dlo = (P.spos ? (long long)__ldg(P.spos + t0) : P.self_first + t0) / SB;
-            dhi = (P.spos ? (long long)__ldg(P.spos + t1) : P.self_first + t1) / SB;
+            dlo = (int)((P.spos ? (long long)__ldg(P.spos + t0) : P.self_first + t0) / SB);
+            dhi = (int)((P.spos ? (long long)__ldg(P.spos + t1) : P.self_first + t1) / SB);
         }
 
         int next_blk = LIST ? __ldg(P.list + u) : 0;
@@ -776,28 +820,6 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_panels_kernel(const
         run_epilogue<NP, PHI>(P, acc, tbase, whole, P.ws + (slot * TT_MAX + tid) * 4);
         u += nrun;
     }
-}
-
-/* first float4 (the frame origin) of panel p inside the blocked panel buffer */
-__device__ __forceinline__ long long panel_entry(long long p)
-{
-    return (p / PPB) * SBH_P + 1 + (p % PPB) * PANEL_SLOTS;
-}
-
-/* The two float4 of one quadrature source (see panel_loop): weight w [C], offset (sx, sy, sz) from the frame
- * origin, all in double; rounded once.  a is rounded first and b, c_phi are derived from the ROUNDED a, so that
- * fma(T, a, b) = a (T - s) up to one rounding of b. */
-__device__ __forceinline__ void panel_encode(double w, double sx, double sy, double sz, float4& A, float4& B)
-{
-    if (w == 0.0 || !isfinite(w)) {
-        A = make_float4(0.f, 1.0e17f, 1.0e17f, 1.0e17f);
-        B = make_float4(0.f, 0.f, 0.f, 0.f);
-        return;
-    }
-    const float a = (float)((w > 0.0 ? 1.0 : -1.0) / sqrt(fabs(w)));
-    const double ad = (double)a;
-    A = make_float4(a, (float)(-ad * sx), (float)(-ad * sy), (float)(-ad * sz));
-    B = make_float4((float)(w * fabs(ad)), (float)(ad * ad), (float)w, 0.f);
 }
 
 /* CTA whose unit range contains unit u (ranges are [floor(cU/G), floor((c+1)U/G)) ) */
@@ -1010,14 +1032,26 @@ __device__ void repair_one(const EvalParams& P, const long long i, double (&red)
 __global__ void __launch_bounds__(THREADS) obem_repair_kernel(const EvalParams P)
 {
     __shared__ double red[4][THREADS];
+    __shared__ long long found[THREADS];
+    __shared__ int nfound;
     const unsigned n = *P.bad_count;
     if (n <= BAD_CAP) {
         for (unsigned r = blockIdx.x; r < n; r += gridDim.x) repair_one(P, P.bad_list[r], red);
-    } else {
-        for (long long i = blockIdx.x; i < P.nt; i += gridDim.x) {
-            const float4 o = P.out[i]; /* CTA-uniform */
-            if (!all_finite(o.x, o.y, o.z, o.w)) repair_one(P, i, red);
+        return;
+    }
+    /* the list overflowed: scan the results (coalesced, THREADS targets per CTA and round), repair what is not finite */
+    for (long long base = (long long)blockIdx.x * THREADS; base < P.nt; base += (long long)gridDim.x * THREADS) {
+        if (threadIdx.x == 0) nfound = 0;
+        __syncthreads();
+        const long long i = base + threadIdx.x;
+        if (i < P.nt) {
+            const float4 o = P.out[i];
+            if (!all_finite(o.x, o.y, o.z, o.w)) found[atomicAdd(&nfound, 1)] = i;
         }
+        __syncthreads();
+        const int nf = nfound;
+        for (int r = 0; r < nf; ++r) repair_one(P, found[r], red); /* any order: each target is recomputed alone */
+        __syncthreads();
     }
 }
 
@@ -1670,6 +1704,7 @@ int obem_destroy(obem_ctx* c)
     if (c->d_map_pts) cudaFree(c->d_map_pts);
     obem_near_free(c);
     obem_nn_free(c);
+    obem_multi_free(c);
     obem_geom_free(c);
     if (c->d_ws) cudaFree(c->d_ws);
     if (c->d_trk_ws) cudaFree(c->d_trk_ws);
@@ -1719,6 +1754,7 @@ int obem_set_panels(obem_ctx* c, const float* d_verts, const float* d_sigma, int
         c->launches += 1;
     }
     c->n_pan = n_panels;
+    c->geom_version += 1;
     return obem_near_store_panels(c, d_verts, d_sigma, n_panels, st);
 }
 

@@ -110,6 +110,37 @@ __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem
 
 inline long long ceil_div(long long a, long long b) { return (a + b - 1) / b; }
 
+/* ------------------------------------------------------------------------------------------- */
+/* blocked panel buffer (obem.cu: the panel launch; obem_multi.cu: the multi-sigma launch)       */
+/* ------------------------------------------------------------------------------------------- */
+/* Panel blocks: PPB panels x (1 origin + 7 x 2) float4 = 510 of 512 slots, + header. */
+constexpr int PPB = 34;
+constexpr int PANEL_SLOTS = 15;
+constexpr int SBH_P = 512 + 1;
+constexpr int PANELS_PER_BLOCK = PPB;
+
+/* first float4 (the frame origin) of panel p inside the blocked panel buffer */
+__device__ __forceinline__ long long panel_entry(long long p)
+{
+    return (p / PPB) * SBH_P + 1 + (p % PPB) * PANEL_SLOTS;
+}
+
+/* The two float4 of one quadrature source (see panel_loop): weight w [C], offset (sx, sy, sz) from the frame
+ * origin, all in double; rounded once.  a is rounded first and b, c_phi are derived from the ROUNDED a, so that
+ * fma(T, a, b) = a (T - s) up to one rounding of b. */
+__device__ __forceinline__ void panel_encode(double w, double sx, double sy, double sz, float4& A, float4& B)
+{
+    if (w == 0.0 || !isfinite(w)) {
+        A = make_float4(0.f, 1.0e17f, 1.0e17f, 1.0e17f);
+        B = make_float4(0.f, 0.f, 0.f, 0.f);
+        return;
+    }
+    const float a = (float)((w > 0.0 ? 1.0 : -1.0) / sqrt(fabs(w)));
+    const double ad = (double)a;
+    A = make_float4(a, (float)(-ad * sx), (float)(-ad * sy), (float)(-ad * sz));
+    B = make_float4((float)(w * fabs(ad)), (float)(ad * ad), (float)w, 0.f);
+}
+
 } /* namespace */
 
 /* obem_nn.cu: buffers of the NN approximation (all library-owned, grown on demand) */
@@ -224,6 +255,12 @@ struct obem_ctx {
     float* d_cell_tri = nullptr;  /* [2 n_cells][3][3] triangles of the polygonal cells */
     float* d_cell_sig = nullptr;  /* [2 n_cells] */
     size_t cell_tri_cap = 0, cell_sig_cap = 0;
+    /* obem_multi.cu: multi-sigma panel evaluation */
+    long long geom_version = 0;  /* incremented by every obem_set_panels */
+    float4* d_munit = nullptr;   /* blocked panel buffer encoded with sigma = 1 (bare weights A_p w_k) */
+    float* d_msig = nullptr;     /* one pass's density vectors, blocked */
+    size_t munit_cap = 0, msig_cap = 0;
+    long long munit_geom = -1;   /* geom_version d_munit was built for */
     /* obem_map.cu */
     float4* d_map_pts = nullptr; /* node coordinates of the last obem_field_map */
     size_t map_pts_cap = 0;      /* bytes */
@@ -295,6 +332,7 @@ int obem_eval_exact(obem_ctx* c, const float4* tgt, long long nt, float4* out, u
 void obem_near_free(obem_ctx* c);
 
 void obem_nn_free(obem_ctx* c);
+void obem_multi_free(obem_ctx* c);
 /* obem_geom.cu */
 int obem_eval_symmetric(obem_ctx* c, const float4* tgt, long long nt, float4* out, unsigned flags, long long self_first,
                         float eps_nbody, cudaStream_t st, float2* trk_out);

@@ -83,11 +83,53 @@ def test_unsoftened_coincident_and_on_quadrature_point(torch_cuda, api, ctx, ref
     ctx.set_softening(0.0, 0.0)
     ctx.set_charges(dev(torch_cuda, xyzq))
     g_n = ctx.eval_at_charges(flags=api.NBODY).cpu().numpy()
-    on, _ = ref.eval_field(xyzq=xyzq, verts=verts, sigma=sigma, eps_pp=0.0)
+    on, op = ref.eval_field(xyzq=xyzq, verts=verts, sigma=sigma, eps_pp=0.0)
     assert np.isfinite(g_n).all()
     assert_parity(g_n, on, "eps=0 nbody with coincident pair")
+    # the panel branch of the repair pass: the zero-distance quadrature point contributes 0 and the VALUE is the
+    # oracle's (the other 6 points of that panel and all other panels)
     g_p = ctx.eval_at_charges(flags=api.PANELS).cpu().numpy()
-    assert np.isfinite(g_p).all()   # the zero-distance quadrature point contributed 0, not inf/nan
+    assert np.isfinite(g_p).all()
+    assert_parity(g_p, op, "eps=0 panels with a charge on a quadrature point")
+    g_b = ctx.eval_at_charges(flags=api.NBODY | api.PANELS).cpu().numpy()
+    assert_parity(g_b, on + op, "eps=0 both, two repaired targets")
+    # the same through eval_at_points: a free point (a field-map node) exactly on that quadrature point, another
+    # exactly on a charge (no index exclusion there: zero distance contributes 0)
+    pts = xyzq[25:40].copy()
+    pts[3, :3] = xyzq[10, :3]
+    g_q = ctx.eval_at_points(dev(torch_cuda, pts), flags=api.NBODY | api.PANELS).cpu().numpy()
+    qn, qp = ref.eval_field(xyzq=xyzq, verts=verts, sigma=sigma, targets=pts, self_index=None, eps_pp=0.0)
+    assert np.isfinite(g_q).all()
+    assert_parity(g_q, qn + qp, "eps=0 points on a quadrature point / on a charge")
+
+
+def test_unsoftened_coincident_pair_through_the_nn_path(torch_cuda, api, ctx, ref):
+    """LIST branch of the repair pass: obem_eval_at_charges_nn at eps = 0 with two different charges at one position.
+    theta = 0 makes the NN sum the exact sum, so the plain oracle applies."""
+    xyzq, _, _ = small_problem(seed=14, n=3000, npan=0)
+    xyzq[100, :3] = xyzq[2900, :3]
+    xyzq[7, :3] = xyzq[8, :3]
+    ctx.set_softening(0.0, 0.0)
+    ctx.set_nn_theta(0.0)
+    ctx.set_charges(dev(torch_cuda, xyzq))
+    g = ctx.eval_at_charges_nn(flags=api.NBODY).cpu().numpy()
+    on, _ = ref.eval_field(xyzq=xyzq, eps_pp=0.0, flags=ref.NBODY)
+    assert np.isfinite(g).all()
+    assert_parity(g, on, "eps=0 NN path (theta = 0) with coincident pairs")
+
+
+def test_more_bad_targets_than_the_repair_list_holds(torch_cuda, api, ctx, ref):
+    """eval_at_points at the charges' own positions with eps = 0: EVERY target sits on a source.  The repair list
+    (2^16 entries) cannot overflow silently: beyond it the pass scans the results for non-finite values.  70,000
+    targets overflow it; sampled values are the oracle's and nothing is left inf/NaN."""
+    xyzq, _, _ = small_problem(seed=15, n=70000, npan=0)
+    ctx.set_softening(0.0, 0.0)
+    ctx.set_charges(dev(torch_cuda, xyzq))
+    g = ctx.eval_at_points(dev(torch_cuda, xyzq), flags=api.NBODY).cpu().numpy()
+    assert np.isfinite(g).all()
+    idx = np.sort(np.random.default_rng(15).choice(70000, 2000, replace=False))
+    on, _ = ref.eval_field(xyzq=xyzq, targets=xyzq[idx], self_index=None, eps_pp=0.0, flags=ref.NBODY)
+    assert_parity(g[idx], on, "every target on a source")
 
 
 def test_softened_coincident_pair_phi(torch_cuda, api, ctx, ref):
