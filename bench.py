@@ -445,7 +445,7 @@ def run_ours(args):
 
     # ---- supplementary, N = 1 only: the adjacent steps, each against its own roofline ----
     if world == 1 and not args.no_next:
-        extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev)
+        extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev, extras["panels_only"]["s"])
         extras["next2"] = bench_next2(torch, api, ctx, wl, timed, dev, extras["nbody_only"]["s"])
         extras["next3"] = bench_next3(torch, api, ctx, wl, timed, out, extras["panels_only"]["s"])
         extras["next4"] = bench_next4(torch, api, ctx, wl, timed, dev)
@@ -650,7 +650,7 @@ def hbm_peak_gbs():
         return 6650.0, "of fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def bench_next1(torch, api, ctx, wl, timed, dev):
+def bench_next1(torch, api, ctx, wl, timed, dev, t_panels):
     """Influence of the particles on the cells (Eq 3.3/3.4; FP32-pipe bound like the hot path), sigma = M^-1 b
     (HBM bound: 4 n^2 bytes read once) and the chained dynamic update, on the bench workload."""
     n, npan = wl.n_charges, wl.n_panels
@@ -660,6 +660,19 @@ def bench_next1(torch, api, ctx, wl, timed, dev):
     res = {"influence": {"s": t_inf, "Ginteractions_per_s": inter / t_inf / 1e9,
                          "frac_fp32_peak": FLOP_PER_INTERACTION * inter / t_inf / 1e12 / peak_flops,
                          "bound": "alu"}}
+    # weighting fields (Eq 3.13): 4 density vectors on the same cells in one pass, against one single-sigma launch
+    gen0 = torch.Generator(device=dev)
+    gen0.manual_seed(1)
+    sig4 = torch.empty((4, npan), dtype=torch.float32, device=dev).normal_(0.0, 1e-5, generator=gen0)
+    pts = torch.from_numpy(wl.xyzq).to(dev)
+    out4 = torch.empty((4, n, 4), dtype=torch.float32, device=dev)
+    t_m4 = timed(lambda: ctx.eval_panels_multi(sig4, pts, out=out4))
+    res["panels_multi_4"] = {"s": t_m4, "vectors": 4, "vs_one_single_sigma_launch": t_m4 / t_panels,
+                             "packed_fp32_instr_per_panel_and_target_pair": {"multi_4": 103, "single": 87},
+                             "Ginteractions_per_s_per_vector_equivalent": 4 * inter / t_m4 / 1e9,
+                             "frac_fp32_peak_of_executed_work": FLOP_PER_INTERACTION * inter * (103.0 / 87.0) / t_m4 / 1e12
+                             / peak_flops, "bound": "alu"}
+    del sig4, out4, pts
     free, _ = torch.cuda.mem_get_info()
     ng = npan
     while ng > 1024 and 4 * ng * ng > 0.6 * free:

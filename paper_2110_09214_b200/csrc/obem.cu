@@ -48,6 +48,10 @@ namespace {
 #ifndef OBEM_DEPTH
 #define OBEM_DEPTH 3 /* re-swept after the per-section split: 1..8 -> 418.1 415.0 412.7 420.5 413.1 413.1 - 413.1 ms (N-body, config 3) */
 #endif
+#ifndef OBEM_PHI_PARTS
+#define OBEM_PHI_PARTS 4 /* separate fp32 phi chains per uniform 256-source block */
+#endif
+constexpr int PHI_PARTS = OBEM_PHI_PARTS;
 constexpr int THREADS = OBEM_THREADS;  /* threads per CTA of the evaluation kernel                 */
 constexpr int TPT = OBEM_TPT;         /* targets per thread                                        */
 constexpr int NPAIR = TPT / 2;        /* packed f32x2 target pairs per thread                      */
@@ -155,7 +159,7 @@ __device__ __forceinline__ long long unit_begin(long long c, long long U, long l
 /*
  * The interaction body, split in two halves so that the loops below can software-pipeline it:
  *   front: 3 FADD2 (d = r_t - r_s), 3 FFMA2 (r2 = d.d + eps^2), 2 MUFU.RSQ
- *   back : FMUL2 (t = w u), FADD2 (phi += t), FMUL2 (u^2), FMUL2 (s = t u^2), 3 FFMA2 (E += s d)
+ *   back (written out in the loops): FMUL2 (t = w u), FADD2 (phi += t), FMUL2 (u^2), FMUL2 (s = t u^2), 3 FFMA2 (E += s d)
  * = 13 packed FP32-pipe instructions + 2 MUFU per (source, target pair).
  * GUARD (eps = 0 only): a source at zero distance contributes 0 (reading A4).
  */
@@ -197,22 +201,9 @@ __device__ __forceinline__ float min_nonneg(float a, float b)
 {
     return __int_as_float(min(__float_as_int(a), __float_as_int(b)));
 }
-template <bool PHI>
-__device__ __forceinline__ void item_back(const u64 dx, const u64 dy, const u64 dz, const u64 u, const u64 w,
-                                          u64& ax, u64& ay, u64& az, u64& ap)
-{
-    const u64 t = mul2(u, w);
-    if (PHI) ap = add2(ap, t);
-    const u64 u2 = mul2(u, u);
-    const u64 sE = mul2(t, u2);
-    ax = fma2(sE, dx, ax);
-    ay = fma2(sE, dy, ay);
-    az = fma2(sE, dz, az);
-}
-
 /* One block of SB point sources against the thread's TPT targets (KIND_POINTS).  Unguarded: see the
  * "speculative zero-distance handling" note at obem_repair_kernel. */
-template <bool TRACK, bool PHI>
+template <bool TRACK, bool PHI, int NS>
 __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                            u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
@@ -220,11 +211,11 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR; /* work items (source, target pair) per trip */
 #pragma unroll 1
-    for (int j0 = 0; j0 < SB; j0 += UNR) {
+    for (int j0 = 0; j0 < NS; j0 += UNR) {
         float4 q[UNR];
 #pragma unroll
         for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j]; /* warp-uniform address: broadcast LDS.128 */
-        u64 dX[K], dY[K], dZ[K], U[K];
+        u64 dX[K], dY[K], dZ[K], U[K], W[K], T[NPAIR];
         /* software pipeline over the K items of the trip: item k's distance + rsqrt are issued DEPTH
          * items before its accumulation, so the MUFU latency is covered by independent FFMA2 work */
 #pragma unroll
@@ -243,32 +234,41 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
-                item_back<PHI>(dX[kk], dY[kk], dZ[kk], U[kk], pk(q[j].w, q[j].w), aX[p], aY[p], aZ[p], aP[p]);
+                /* as item_back, with phi summed as a tree over the 4 sources of the trip (see block_loop_uniform) */
+                W[kk] = mul2(U[kk], pk(q[j].w, q[j].w));
+                if (PHI && j == 1) T[p] = add2(W[kk - NPAIR], W[kk]);
+                if (PHI && j == 3) aP[p] = add2(aP[p], add2(T[p], add2(W[kk - NPAIR], W[kk])));
+                const u64 sE = mul2(W[kk], mul2(U[kk], U[kk]));
+                aX[p] = fma2(sE, dX[kk], aX[p]);
+                aY[p] = fma2(sE, dY[kk], aY[p]);
+                aZ[p] = fma2(sE, dZ[kk], aZ[p]);
             }
         }
     }
 }
 
-/* Statement-order knobs of the uniform loop.  ptxas schedules the ~235-instruction trip itself, and on two warps per
- * SM sub-partition the result decides +-3 % of the launch (measured: 420 .. 447 ms on config 3 over 36 orders that
- * differ in nothing else), so the order is a tuned parameter per instantiation -- VE: order of the three E FMAs,
- * VP: where the phi add sits, D: pipeline distance, VF: order of the r2 FMAs.  DESIGN.md section 5 has the sweep. */
+/* Statement-order knobs of the uniform loop.  ptxas schedules the ~235-instruction trip itself, and with two warps per
+ * SM sub-partition the schedule it finds decides +-3 % of the launch (measured on config 3: 418.5 .. 447.4 ms over
+ * 216 orders that differ in nothing else), so the order is a tuned parameter per instantiation -- D: pipeline
+ * distance, VE: order of the three E FMAs, VP: where the phi add sits, VF: order of the three r2 FMAs.  VF changes
+ * the rounding of r2, so it is the SAME in all instantiations (E of the E-only and of the partner-tracking launch
+ * stays bit-identical to the plain launch); the others are free.  DESIGN.md section 5 has the sweep. */
 /* each knob set is four decimal digits: D, VE, VP, VF */
 #ifndef OBEM_KNOBS_PHI
-#define OBEM_KNOBS_PHI 4220
+#define OBEM_KNOBS_PHI 5201
 #endif
 #ifndef OBEM_KNOBS_E
-#define OBEM_KNOBS_E 5300
+#define OBEM_KNOBS_E 6201
 #endif
 #ifndef OBEM_KNOBS_T
-#define OBEM_KNOBS_T 3000
+#define OBEM_KNOBS_T 5201
 #endif
 /* the same for the panel loop (VF unused) */
 #ifndef OBEM_PKNOBS_PHI
 #define OBEM_PKNOBS_PHI 5200
 #endif
 #ifndef OBEM_PKNOBS_E
-#define OBEM_PKNOBS_E 5200
+#define OBEM_PKNOBS_E 6300
 #endif
 struct Knobs {
     int d, ve, vp, vf;
@@ -276,6 +276,7 @@ struct Knobs {
 constexpr Knobs knobs_of(int code) { return Knobs{code / 1000, (code / 100) % 10, (code / 10) % 10, code % 10}; }
 constexpr Knobs KNOBS_PHI = knobs_of(OBEM_KNOBS_PHI), KNOBS_E = knobs_of(OBEM_KNOBS_E), KNOBS_T = knobs_of(OBEM_KNOBS_T);
 constexpr Knobs PKNOBS_PHI = knobs_of(OBEM_PKNOBS_PHI), PKNOBS_E = knobs_of(OBEM_PKNOBS_E);
+static_assert(KNOBS_PHI.vf == KNOBS_E.vf && KNOBS_PHI.vf == KNOBS_T.vf, "VF changes the rounding of r2: one value for all");
 
 template <int VF>
 __device__ __forceinline__ void uni_front(u64& dx, u64& dy, u64& dz, u64& u, float& r2l, float& r2h, const u64 tx,
@@ -297,11 +298,12 @@ __device__ __forceinline__ void uni_front(u64& dx, u64& dy, u64& dz, u64& u, flo
 }
 
 /*
- * Same for a block whose SB sources all carry the weight w (header): sum_j w f(r_j) = w sum_j f(r_j), so the
- * weight is applied once per block and the body is 12 packed instructions: phi += u, u^2, u^3, E += u^3 d.
+ * NS sources of a block whose SB sources all carry the weight w (header): sum_j w f(r_j) = w sum_j f(r_j), so the
+ * weight is applied once per block (by the caller) and the body is 12 packed instructions: phi += u, u^2, u^3,
+ * E += u^3 d.
  */
-template <bool TRACK, bool PHI>
-__device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2, const float w,
+template <bool TRACK, bool PHI, int NS>
+__device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2,
                                                    const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
                                                    u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
@@ -310,12 +312,21 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
     constexpr int DEPTH = KN.d;
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR;
+    static_assert(UNR == 4, "the phi tree below sums the 4 sources of a trip");
 #pragma unroll 1
-    for (int j0 = 0; j0 < SB; j0 += UNR) {
+    for (int j0 = 0; j0 < NS; j0 += UNR) {
         float4 q[UNR];
 #pragma unroll
         for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j];
         u64 dX[K], dY[K], dZ[K], U[K];
+        u64 T[NPAIR];
+        /* phi: the 4 values of a trip are summed as a tree, (u0 + u1) + (u2 + u3), and the running sum takes one add
+         * per trip -- the same 4 adds per 4 sources, but the long fp32 chain is 4x shorter */
+#define OBEM_PHI_TERM()                                                                         \
+    do {                                                                                        \
+        if ((kk / NPAIR) == 1) T[p] = add2(U[kk - NPAIR], U[kk]);                               \
+        if ((kk / NPAIR) == 3) aP[p] = add2(aP[p], add2(T[p], add2(U[kk - NPAIR], U[kk])));     \
+    } while (0)
 #pragma unroll
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
@@ -331,25 +342,18 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
             }
             if (k >= DEPTH) {
                 const int kk = k - DEPTH, p = kk % NPAIR;
-                if (PHI && KN.vp == 0) aP[p] = add2(aP[p], U[kk]);
+                if (PHI && KN.vp == 0) OBEM_PHI_TERM();
                 const u64 u2 = mul2(U[kk], U[kk]);
                 const u64 u3 = mul2(u2, U[kk]);
-                if (PHI && KN.vp == 1) aP[p] = add2(aP[p], U[kk]);
+                if (PHI && KN.vp == 1) OBEM_PHI_TERM();
                 if (KN.ve == 0) { aX[p] = fma2(u3, dX[kk], aX[p]); aY[p] = fma2(u3, dY[kk], aY[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); }
                 if (KN.ve == 1) { aZ[p] = fma2(u3, dZ[kk], aZ[p]); aY[p] = fma2(u3, dY[kk], aY[p]); aX[p] = fma2(u3, dX[kk], aX[p]); }
                 if (KN.ve == 2) { aY[p] = fma2(u3, dY[kk], aY[p]); aX[p] = fma2(u3, dX[kk], aX[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); }
                 if (KN.ve == 3) { aX[p] = fma2(u3, dX[kk], aX[p]); aZ[p] = fma2(u3, dZ[kk], aZ[p]); aY[p] = fma2(u3, dY[kk], aY[p]); }
-                if (PHI && KN.vp == 2) aP[p] = add2(aP[p], U[kk]);
+                if (PHI && KN.vp == 2) OBEM_PHI_TERM();
             }
         }
-    }
-    const u64 w2 = pk(w, w);
-#pragma unroll
-    for (int p = 0; p < NPAIR; ++p) {
-        aX[p] = mul2(aX[p], w2);
-        aY[p] = mul2(aY[p], w2);
-        aZ[p] = mul2(aZ[p], w2);
-        if (PHI) aP[p] = mul2(aP[p], w2);
+#undef OBEM_PHI_TERM
     }
 }
 
@@ -441,34 +445,51 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
  * source index of the block), or -1 if that target is not in this block; always guarded (d = 0 there).
  * Simple loop: it runs for ~TT/SB of the blocks of a tile only.
  */
-template <bool TRACK, bool PHI>
+template <bool TRACK, bool PHI, int NS>
 __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                              const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                              u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR],
-                                             const int (&rel)[TPT], float (&bm)[TPT],
+                                             const int (&rel)[TPT], const int joff, float (&bm)[TPT],
                                              const unsigned negmask, const unsigned posmask)
 {
     const u64 e2 = pk(eps2, eps2);
+    static_assert(NS % 4 == 0, "phi is summed as a tree over groups of 4 sources, as in block_loop");
 #pragma unroll 1
-    for (int j = 0; j < SB; ++j) {
-        const float4 q = s[j];
+    for (int j0 = 0; j0 < NS; j0 += 4) {
+        u64 W[4][NPAIR];
 #pragma unroll
-        for (int p = 0; p < NPAIR; ++p) {
-            u64 dx, dy, dz, u;
-            if (TRACK) {
-                /* TRACK also sends every non-uniform block here: the sign is tested per source.  The self term has
-                 * the target's own sign, so it is never a partner. */
-                const unsigned el = (q.w > 0.f) ? negmask : ((q.w < 0.f) ? posmask : 0u);
-                float r2l, r2h;
-                item_front_r2<true>(dx, dy, dz, u, r2l, r2h, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
-                if ((el >> (2 * p)) & 1u) bm[2 * p] = min_nonneg(bm[2 * p], r2l);
-                if ((el >> (2 * p + 1)) & 1u) bm[2 * p + 1] = min_nonneg(bm[2 * p + 1], r2h);
-            } else {
-                item_front<true>(dx, dy, dz, u, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+        for (int g = 0; g < 4; ++g) {
+            const float4 q = s[j0 + g];
+            const int j = joff + j0 + g; /* index of the source inside its block */
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p) {
+                u64 dx, dy, dz, u;
+                if (TRACK) {
+                    /* TRACK also sends the blocks of mixed sign here: the sign is tested per source.  The self term
+                     * has the target's own sign, so it is never a partner. */
+                    const unsigned el = (q.w > 0.f) ? negmask : ((q.w < 0.f) ? posmask : 0u);
+                    float r2l, r2h;
+                    item_front_r2<true>(dx, dy, dz, u, r2l, r2h, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+                    if ((el >> (2 * p)) & 1u) bm[2 * p] = min_nonneg(bm[2 * p], r2l);
+                    if ((el >> (2 * p + 1)) & 1u) bm[2 * p + 1] = min_nonneg(bm[2 * p + 1], r2h);
+                } else {
+                    item_front<true>(dx, dy, dz, u, X[p], Y[p], Z[p], q.x, q.y, q.z, e2);
+                }
+                const float wl = (rel[2 * p] == j) ? 0.0f : q.w;
+                const float wh = (rel[2 * p + 1] == j) ? 0.0f : q.w;
+                /* the same operations in the same order as block_loop's back half: a block that takes this loop in
+                 * one instantiation and block_loop in another gives the same bits */
+                W[g][p] = mul2(u, pk(wl, wh));
+                const u64 sE = mul2(W[g][p], mul2(u, u));
+                aX[p] = fma2(sE, dx, aX[p]);
+                aY[p] = fma2(sE, dy, aY[p]);
+                aZ[p] = fma2(sE, dz, aZ[p]);
             }
-            const float wl = (rel[2 * p] == j) ? 0.0f : q.w;
-            const float wh = (rel[2 * p + 1] == j) ? 0.0f : q.w;
-            item_back<PHI>(dx, dy, dz, u, pk(wl, wh), aX[p], aY[p], aZ[p], aP[p]);
+        }
+        if (PHI) {
+#pragma unroll
+            for (int p = 0; p < NPAIR; ++p)
+                aP[p] = add2(aP[p], add2(add2(W[0][p], W[1][p]), add2(W[2][p], W[3][p])));
         }
     }
 }
@@ -681,6 +702,26 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
 #pragma unroll
                 for (int k = 0; k < TPT; ++k) bm[k] = __int_as_float(0x7f800000);
             }
+            /* phi: PHI_PARTS separate fp32 chains over the block's sources, joined after the block.  Within a block the
+             * terms (nearly) all have one sign, so the chain length sets the rounding error;
+             * E: one chain */
+            constexpr int PARTS = PHI ? PHI_PARTS : 1;
+            constexpr int NSP = SB / PARTS;
+            u64 aQ[PARTS > 1 ? PARTS - 1 : 1][NPAIR];
+#pragma unroll
+            for (int h = 0; h < PARTS - 1; ++h)
+#pragma unroll
+                for (int p = 0; p < NPAIR; ++p) aQ[h][p] = 0ull;
+            static_assert(PHI_PARTS == 1 || PHI_PARTS == 2 || PHI_PARTS == 4, "phi_join below");
+            auto phi_join = [&]() {
+                if (PHI) {
+#pragma unroll
+                    for (int p = 0; p < NPAIR; ++p) {
+                        if (PARTS == 4) aP[p] = add2(add2(aP[p], aQ[0][p]), add2(aQ[PARTS > 2 ? 1 : 0][p], aQ[PARTS > 2 ? 2 : 0][p]));
+                        if (PARTS == 2) aP[p] = add2(aP[p], aQ[0][p]);
+                    }
+                }
+            };
             bool diag = (!LIST || blk < P.list_self_blocks) && blk >= dlo && blk <= dhi;
             if (diag && P.spos) { /* CTA-uniform branch: inside the hull, does any target really live in blk? */
                 int mine = 0;
@@ -703,12 +744,30 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
                     if (diag && i < P.nt) rr = (P.spos ? (long long)__ldg(P.spos + i) : P.self_first + i) - blk * SB;
                     rel[k] = (rr >= 0 && rr < SB) ? (int)rr : -1;
                 }
-                self_block_loop<TRACK, PHI>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, rel, bm, negmask, posmask);
+#pragma unroll
+                for (int h = 0; h < PARTS; ++h)
+                    self_block_loop<TRACK, PHI, NSP>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0],
+                                                     rel, h * NSP, bm, negmask, posmask);
+                phi_join();
             } else if (blkw == blkw) {
-                block_loop_uniform<TRACK, PHI>(sblk, eps2, blkw, X, Y, Z, aX, aY, aZ, aP, bm);
+#pragma unroll
+                for (int h = 0; h < PARTS; ++h)
+                    block_loop_uniform<TRACK, PHI, NSP>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
+                phi_join();
+                const u64 w2 = pk(blkw, blkw);
+#pragma unroll
+                for (int p = 0; p < NPAIR; ++p) {
+                    aX[p] = mul2(aX[p], w2);
+                    aY[p] = mul2(aY[p], w2);
+                    aZ[p] = mul2(aZ[p], w2);
+                    if (PHI) aP[p] = mul2(aP[p], w2);
+                }
                 elig = (blkw > 0.f) ? negmask : ((blkw < 0.f) ? posmask : 0u);
             } else {
-                block_loop<TRACK, PHI>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, bm);
+#pragma unroll
+                for (int h = 0; h < PARTS; ++h)
+                    block_loop<TRACK, PHI, NSP>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
+                phi_join();
                 elig = (blks > 0.f) ? negmask : ((blks < 0.f) ? posmask : 0u);
             }
             if (TRACK) {

@@ -3,16 +3,19 @@
 For E:   rel-L2 = sqrt(sum_t ||dE_t||^2 / sum_t ||E_ref,t||^2)            bar 2e-5
          per-target max of ||dE_t|| / ||E_ref,t||                         bar 1e-3
 For phi: rel-L2 over all phi                                              bar 2e-5
-         per-target |dphi| / max(|phi_ref|, 0.1 * rms(phi_ref))           bar 1e-3
+         per-target |dphi| / max(|phi_ref|, PHI_FLOOR * rms(phi_ref))     bar 1e-3,  PHI_FLOOR = 1e-2
 (phi changes sign inside a neutral cloud: it is a small difference of two large sums, the electrons' and the
-ions', so "relative to |phi_t|" is meaningless where phi_t crosses zero.  A target whose |phi| is below 10 % of
-the rms is measured against 10 % of the rms.  DESIGN.md reading A6 derives the floor from the arithmetic: fp32
-two-level accumulation with an exactly rounded rsqrt already errs by 2e-5 * rms on config 1.)
+ions', so "relative to |phi_t|" is meaningless where phi_t crosses zero.  A target whose |phi| is below 1 % of the rms
+is measured against 1 % of the rms.  Round 1 needed a floor of 10 % of the rms; the fp64 running sums and the short
+fp32 phi chains of round 2 brought the measured worst case at a 1 % floor to 5e-4 (N-body part
+of config 2).  SURVEY.md's first proposal, 0.1 % of the rms, asks for an absolute error of 1e-6 rms on sums whose
+terms add up to ~50 rms in fp32: section 7 gives the bound that says why that is out of reach.)
 """
 import numpy as np
 
 TOL_REL_L2 = 2e-5
 TOL_MAX_REL = 1e-3
+PHI_FLOOR = 1e-2
 
 
 def field_errors(got, ref):
@@ -31,7 +34,7 @@ def field_errors(got, ref):
     dphi = got[:, 3] - ref[:, 3]
     rms = float(np.sqrt((ref[:, 3] ** 2).mean()))
     p_l2 = float(np.sqrt((dphi ** 2).sum() / max((ref[:, 3] ** 2).sum(), 1e-300)))
-    p_max = float((np.abs(dphi) / np.maximum(np.abs(ref[:, 3]), max(0.1 * rms, 1e-300))).max())
+    p_max = float((np.abs(dphi) / np.maximum(np.abs(ref[:, 3]), max(PHI_FLOOR * rms, 1e-300))).max())
     return {"E_rel_l2": e_l2, "E_max_rel": e_max, "phi_rel_l2": p_l2, "phi_max_rel": p_max}
 
 
