@@ -241,8 +241,8 @@ int obem_step_pefrl(obem_ctx* c, float* d_xyzq, float* d_vel, int64_t n, float d
  *   d_partner_d [count] fp32 = true (unsoftened) distance [m], +inf if there is none
  *   d_partner_j [count] int32 = index of that charge in the charge set, -1 if there is none
  * Charges with q = 0 have no partner and are nobody's partner.  How: the evaluation kernel keeps, per target, the
- * smallest SOFTENED fp32 r2 over opposite-sign sources and the 256-source block it fell in (2 integer min per packed
- * interaction on the ALU pipe); a second O(256 N) kernel scans that block exactly.  Near-ties between different
+ * smallest SOFTENED fp32 r2 over opposite-sign sources and the 256-source block it fell in (one 3-input integer min
+ * per two sources and target on the ALU pipe); a second O(256 N) kernel scans that block exactly.  Near-ties between different
  * blocks are decided on the fp32 softened r2: the reported distance d obeys d^2 <= d_true^2 + 4 ulp(d_true^2 +
  * eps_pp^2).  A pair recombines when d <= obem_recombination_radius(E_ioni), Eq (3.12). */
 int obem_eval_at_charges_partners(obem_ctx* c, float* d_out, float* d_partner_d, int32_t* d_partner_j,

@@ -201,6 +201,11 @@ __device__ __forceinline__ float min_nonneg(float a, float b)
 {
     return __int_as_float(min(__float_as_int(a), __float_as_int(b)));
 }
+/* the same over three values in ONE instruction (VIMNMX3): two sources per min halve the cost of partner tracking */
+__device__ __forceinline__ float min3_nonneg(float a, float b, float c)
+{
+    return __int_as_float(__vimin3_s32(__float_as_int(a), __float_as_int(b), __float_as_int(c)));
+}
 /* One block of SB point sources against the thread's TPT targets (KIND_POINTS).  Unguarded: see the
  * "speculative zero-distance handling" note at obem_repair_kernel. */
 template <bool TRACK, bool PHI, int NS>
@@ -216,6 +221,7 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
 #pragma unroll
         for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j]; /* warp-uniform address: broadcast LDS.128 */
         u64 dX[K], dY[K], dZ[K], U[K], W[K], T[NPAIR];
+        float R2L[K], R2H[K];
         /* software pipeline over the K items of the trip: item k's distance + rsqrt are issued DEPTH
          * items before its accumulation, so the MUFU latency is covered by independent FFMA2 work */
 #pragma unroll
@@ -223,11 +229,12 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
                 if (TRACK) { /* as in block_loop_uniform: the block is of one sign (header .y), decided after the block */
-                    float r2l, r2h;
-                    item_front_r2<false>(dX[k], dY[k], dZ[k], U[k], r2l, r2h, X[p], Y[p], Z[p], q[j].x, q[j].y,
+                    item_front_r2<false>(dX[k], dY[k], dZ[k], U[k], R2L[k], R2H[k], X[p], Y[p], Z[p], q[j].x, q[j].y,
                                          q[j].z, e2);
-                    bm[2 * p] = min_nonneg(bm[2 * p], r2l);
-                    bm[2 * p + 1] = min_nonneg(bm[2 * p + 1], r2h);
+                    if (j & 1) {
+                        bm[2 * p] = min3_nonneg(bm[2 * p], R2L[k - NPAIR], R2L[k]);
+                        bm[2 * p + 1] = min3_nonneg(bm[2 * p + 1], R2H[k - NPAIR], R2H[k]);
+                    }
                 } else {
                     item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
                 }
@@ -261,7 +268,7 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
 #define OBEM_KNOBS_E 6201
 #endif
 #ifndef OBEM_KNOBS_T
-#define OBEM_KNOBS_T 5201
+#define OBEM_KNOBS_T 3001
 #endif
 /* the same for the panel loop (VF unused) */
 #ifndef OBEM_PKNOBS_PHI
@@ -320,6 +327,7 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
         for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j];
         u64 dX[K], dY[K], dZ[K], U[K];
         u64 T[NPAIR];
+        float R2L[K], R2H[K];
         /* phi: the 4 values of a trip are summed as a tree, (u0 + u1) + (u2 + u3), and the running sum takes one add
          * per trip -- the same 4 adds per 4 sources, but the long fp32 chain is 4x shorter */
 #define OBEM_PHI_TERM()                                                                         \
@@ -331,13 +339,13 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
         for (int k = 0; k < K + DEPTH; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
-                float r2l, r2h;
-                uni_front<KN.vf>(dX[k], dY[k], dZ[k], U[k], r2l, r2h, X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
-                if (TRACK) {
-                    /* by-product: smallest softened r2 of the block per target, 2 VIMNMX on the
-                     * otherwise idle ALU pipe; whether the block's sign is opposite is decided after the block */
-                    bm[2 * p] = min_nonneg(bm[2 * p], r2l);
-                    bm[2 * p + 1] = min_nonneg(bm[2 * p + 1], r2h);
+                uni_front<KN.vf>(dX[k], dY[k], dZ[k], U[k], R2L[k], R2H[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
+                if (TRACK && (j & 1)) {
+                    /* by-product: smallest softened r2 of the block per target -- one 3-input integer
+                     * min (VIMNMX3) per two sources and target on the otherwise idle ALU pipe; whether the block's
+                     * sign is opposite is decided after the block */
+                    bm[2 * p] = min3_nonneg(bm[2 * p], R2L[k - NPAIR], R2L[k]);
+                    bm[2 * p + 1] = min3_nonneg(bm[2 * p + 1], R2H[k - NPAIR], R2H[k]);
                 }
             }
             if (k >= DEPTH) {
