@@ -139,6 +139,7 @@ constexpr unsigned BAD_CAP = 1u << 16;
 /* dynamic shared memory of the evaluation kernels: their fp64 running sums (acc_flush) */
 constexpr size_t ACC_BYTES_POINTS = (size_t)8 * NPAIR * THREADS * sizeof(double);
 constexpr size_t ACC_BYTES_PANELS = (size_t)8 * PANEL_NPAIR * THREADS * sizeof(double);
+constexpr size_t ACC_BYTES_SMALL = (size_t)8 * 1 * THREADS * sizeof(double); /* the small-tile instantiations */
 
 __device__ __forceinline__ bool all_finite(float a, float b, float c, float d)
 {
@@ -208,10 +209,10 @@ __device__ __forceinline__ float min3_nonneg(float a, float b, float c)
 }
 /* One block of SB point sources against the thread's TPT targets (KIND_POINTS).  Unguarded: see the
  * "speculative zero-distance handling" note at obem_repair_kernel. */
-template <bool TRACK, bool PHI, int NS>
+template <bool TRACK, bool PHI, int NS, int NPAIR>
 __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
-                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
+                                           u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[2 * NPAIR])
 {
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR; /* work items (source, target pair) per trip */
@@ -309,11 +310,11 @@ __device__ __forceinline__ void uni_front(u64& dx, u64& dy, u64& dz, u64& u, flo
  * weight is applied once per block (by the caller) and the body is 12 packed instructions: phi += u, u^2, u^3,
  * E += u^3 d.
  */
-template <bool TRACK, bool PHI, int NS>
+template <bool TRACK, bool PHI, int NS, int NPAIR>
 __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2,
                                                    const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
-                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[TPT])
+                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[2 * NPAIR])
 {
     constexpr Knobs KN = TRACK ? KNOBS_T : (PHI ? KNOBS_PHI : KNOBS_E);
     constexpr int DEPTH = KN.d;
@@ -453,11 +454,11 @@ __device__ __forceinline__ void panel_loop(const float4* __restrict__ s, const f
  * source index of the block), or -1 if that target is not in this block; always guarded (d = 0 there).
  * Simple loop: it runs for ~TT/SB of the blocks of a tile only.
  */
-template <bool TRACK, bool PHI, int NS>
+template <bool TRACK, bool PHI, int NS, int NPAIR>
 __device__ __forceinline__ void self_block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                              const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                              u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR],
-                                             const int (&rel)[TPT], const int joff, float (&bm)[TPT],
+                                             const int (&rel)[2 * NPAIR], const int joff, float (&bm)[2 * NPAIR],
                                              const unsigned negmask, const unsigned posmask)
 {
     const u64 e2 = pk(eps2, eps2);
@@ -593,9 +594,10 @@ __device__ __forceinline__ void run_epilogue(const EvalParams& P, const double* 
  * integrators read only E, PAPER.md:302-306 -- one packed instruction of 12 less).  One instantiation per variant:
  * each hot loop gets its own register allocation.
  */
-template <bool TRACK, bool LIST, bool PHI>
+template <bool TRACK, bool LIST, bool PHI, int NPAIR>
 __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const EvalParams P)
 {
+    constexpr int TPT = 2 * NPAIR, TT = THREADS * TPT; /* targets per thread and per tile of THIS instantiation */
     static_assert(!LIST || !TRACK, "LIST mode: no partner tracking");
     extern __shared__ __align__(16) double acc_dyn[]; /* [8 NPAIR][THREADS] running sums, fp64 */
     __shared__ __align__(128) float4 ring[STAGES][SBH + 3]; /* stage stride % 64 B == 0 */
@@ -713,7 +715,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             /* phi: PHI_PARTS separate fp32 chains over the block's sources, joined after the block.  Within a block the
              * terms (nearly) all have one sign, so the chain length sets the rounding error;
              * E: one chain */
-            constexpr int PARTS = PHI ? PHI_PARTS : 1;
+            constexpr int PARTS = (PHI && !LIST) ? PHI_PARTS : 1; /* LIST: the NN approximation errs by 1e-3 anyway */
             constexpr int NSP = SB / PARTS;
             u64 aQ[PARTS > 1 ? PARTS - 1 : 1][NPAIR];
 #pragma unroll
@@ -754,13 +756,13 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
                 }
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)
-                    self_block_loop<TRACK, PHI, NSP>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0],
+                    self_block_loop<TRACK, PHI, NSP, NPAIR>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0],
                                                      rel, h * NSP, bm, negmask, posmask);
                 phi_join();
             } else if (blkw == blkw) {
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)
-                    block_loop_uniform<TRACK, PHI, NSP>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
+                    block_loop_uniform<TRACK, PHI, NSP, NPAIR>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
                 phi_join();
                 const u64 w2 = pk(blkw, blkw);
 #pragma unroll
@@ -774,7 +776,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             } else {
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)
-                    block_loop<TRACK, PHI, NSP>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
+                    block_loop<TRACK, PHI, NSP, NPAIR>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
                 phi_join();
                 elig = (blks > 0.f) ? negmask : ((blks < 0.f) ? posmask : 0u);
             }
@@ -1585,19 +1587,39 @@ int obem_eval_internal(obem_ctx* c, const float4* tgt, long long nt, float4* out
                 Q.self_first = 0;
             }
         }
+        /* Small problems: a work unit (tile x block) of the big tiles is ~29 us of FP32 work whatever the problem
+         * size, so a problem of fewer units than 3/4 of the grid leaves most SMs idle for that long.  It runs the
+         * small-tile instantiations instead (2 targets per thread: 4-5 x more, shorter units). */
+        const bool small_tiles = 4 * Q.ntiles * Q.nblk <= 3LL * c->grid;
+        if (small_tiles) {
+            Q.tpt = 2;
+            Q.tt = 2 * THREADS;
+            Q.ws_stride = Q.tt; /* the partner workspace is indexed with the instantiation's own tile size */
+            Q.ntiles = ceil_div(nt, (long long)Q.tt);
+        }
         Q.U = Q.ntiles * Q.nblk;
         Q.accumulate = (k > 0);
         if (Q.sec[0].kind == KIND_PANELS) {
             Q.self_first = -1;
             Q.trk_out = nullptr;
-            if (phi) obem_panels_kernel<PANEL_NPAIR, true><<<c->grid, THREADS, ACC_BYTES_PANELS, st>>>(Q);
-            else obem_panels_kernel<PANEL_NPAIR, false><<<c->grid, THREADS, ACC_BYTES_PANELS, st>>>(Q);
+            if (small_tiles) {
+                if (phi) obem_panels_kernel<1, true><<<c->grid, THREADS, ACC_BYTES_SMALL, st>>>(Q);
+                else obem_panels_kernel<1, false><<<c->grid, THREADS, ACC_BYTES_SMALL, st>>>(Q);
+            } else if (phi) {
+                obem_panels_kernel<PANEL_NPAIR, true><<<c->grid, THREADS, ACC_BYTES_PANELS, st>>>(Q);
+            } else {
+                obem_panels_kernel<PANEL_NPAIR, false><<<c->grid, THREADS, ACC_BYTES_PANELS, st>>>(Q);
+            }
+        } else if (small_tiles) {
+            if (Q.trk_out) obem_eval_kernel<true, false, true, 1><<<c->grid, THREADS, ACC_BYTES_SMALL, st>>>(Q);
+            else if (phi) obem_eval_kernel<false, false, true, 1><<<c->grid, THREADS, ACC_BYTES_SMALL, st>>>(Q);
+            else obem_eval_kernel<false, false, false, 1><<<c->grid, THREADS, ACC_BYTES_SMALL, st>>>(Q);
         } else if (Q.trk_out) {
-            obem_eval_kernel<true, false, true><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
+            obem_eval_kernel<true, false, true, NPAIR><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
         } else if (phi) {
-            obem_eval_kernel<false, false, true><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
+            obem_eval_kernel<false, false, true, NPAIR><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
         } else {
-            obem_eval_kernel<false, false, false><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
+            obem_eval_kernel<false, false, false, NPAIR><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(Q);
         }
         OBEM_CUDA(c, cudaGetLastError());
         obem_fixup_kernel<<<dim3((unsigned)Q.ntiles, (unsigned)Q.tpt), THREADS, (size_t)(c->grid + 2) * sizeof(long long),
@@ -1659,7 +1681,7 @@ int obem_eval_list(obem_ctx* c, const float4* tgt, long long nt, float4* out, co
     P.bad_count = c->d_bad_count;
     P.bad_list = c->d_bad_list;
     OBEM_CUDA(c, cudaMemsetAsync(c->d_bad_count, 0, sizeof(unsigned), st));
-    obem_eval_kernel<false, true, true><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(P);
+    obem_eval_kernel<false, true, true, NPAIR><<<c->grid, THREADS, ACC_BYTES_POINTS, st>>>(P);
     OBEM_CUDA(c, cudaGetLastError());
     obem_fixup_kernel<<<dim3((unsigned)P.ntiles, (unsigned)P.tpt), THREADS, (size_t)(c->grid + 2) * sizeof(long long), st>>>(
         P, c->grid);
@@ -1711,14 +1733,20 @@ int obem_create(obem_ctx** out, int device)
     c->sm_count = prop.multiProcessorCount;
     int per_sm = 0;
     /* the running sums of the evaluation kernels live in dynamic shared memory beyond the 48 KB default */
-    e = cudaFuncSetAttribute(obem_eval_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    e = cudaFuncSetAttribute(obem_eval_kernel<false, false, true, NPAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, false, false, NPAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<true, false, true, NPAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, true, true, NPAIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_POINTS);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_panels_kernel<PANEL_NPAIR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_PANELS);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_panels_kernel<PANEL_NPAIR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_PANELS);
+    /* the small-tile instantiations: static + dynamic shared memory of the panel ones is just above 48 KB */
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, false, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_SMALL);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<false, false, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_SMALL);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_eval_kernel<true, false, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_SMALL);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_panels_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_SMALL);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(obem_panels_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ACC_BYTES_SMALL);
     if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<true, false, true>, THREADS, ACC_BYTES_POINTS);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, obem_eval_kernel<true, false, true, NPAIR>, THREADS, ACC_BYTES_POINTS);
     if (e != cudaSuccess || per_sm < 1) {
         /* no sm_100a code for this device, or the kernel cannot be resident */
         cudaGetLastError();

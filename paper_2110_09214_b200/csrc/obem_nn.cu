@@ -6,7 +6,7 @@
  *
  *   1. k-d partition with equal-count leaves: level by level, every segment of more than 256 charges is sorted
  *      (stably) along the longest axis of its bounding box and cut at a multiple of 256 -- one radix sort per level
- *      over the whole array with key = (segment start, coordinate).  A leaf = 256 charges = one source block of the
+ *      over the whole array with key = (segment rank, coordinate).  A leaf = 256 charges = one source block of the
  *      evaluation kernel; a target group = 8 consecutive leaves = one 2048-target tile.
  *   2. Per leaf, and per super-leaf (64 consecutive leaves): bounding box and two pseudo-particles (the centres of
  *      charge of its positive and of its negative members).
@@ -40,15 +40,25 @@ __host__ __device__ __forceinline__ long long nn_split(long long a, long long b)
     const long long leaves = (b - a + LEAF - 1) / LEAF;
     return a + (long long)LEAF * ((leaves + 1) / 2);
 }
-/* segment [a, b) that holds position i after `level` rounds of cuts */
-__device__ __forceinline__ void nn_segment(long long n, long long i, int level, long long& a, long long& b)
+/* segment [a, b) that holds position i after `level` rounds of cuts; rank = its `level`-bit path (0 = left, 1 = right
+ * at every cut, 0 once a segment is final): ascending in position, so it can stand for the segment in a sort key */
+__device__ __forceinline__ void nn_segment(long long n, long long i, int level, long long& a, long long& b,
+                                           unsigned& rank)
 {
     a = 0, b = n;
-    for (int t = 0; t < level && b - a > LEAF; ++t) {
+    rank = 0u;
+    for (int t = 0; t < level; ++t) {
+        rank <<= 1;
+        if (b - a <= LEAF) continue;
         const long long m = nn_split(a, b);
         if (i < m) b = m;
-        else a = m;
+        else a = m, rank |= 1u;
     }
+}
+__device__ __forceinline__ void nn_segment(long long n, long long i, int level, long long& a, long long& b)
+{
+    unsigned rank;
+    nn_segment(n, i, level, a, b, rank);
 }
 /* fp32 bits -> unsigned whose order is the IEEE total order of the floats */
 __device__ __forceinline__ unsigned nn_ordered(float f)
@@ -145,7 +155,8 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     long long a, b;
-    nn_segment(n, i, level, a, b);
+    unsigned rank;
+    nn_segment(n, i, level, a, b, rank);
     unsigned low;
     if (b - a <= LEAF) {
         low = (unsigned)(i - a); /* keep the order of a final segment */
@@ -160,7 +171,7 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
         const float4 p = x[perm[i]];
         low = nn_ordered(ax == 0 ? p.x : (ax == 1 ? p.y : p.z));
     }
-    keys[i] = ((u64k)(a / LEAF) << 32) | (u64k)low; /* segment starts are multiples of LEAF: fewer key bits to sort */
+    keys[i] = ((u64k)rank << 32) | (u64k)low; /* `level` bits of segment rank + 32 of coordinate: 4-6 radix passes */
 }
 
 /* one CTA per leaf: sorted copy (plain, padded) + blocked copy with header + bounding box + the two pseudo-particles */
@@ -501,7 +512,7 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
         nn_key_kernel<<<gn, 256, 0, st>>>(c->d_chg, S.perm[cur], n, level, segmin, segmax, S.key[cur]);
         OBEM_CUDA(c, cudaGetLastError());
         OBEM_CUDA(c, cub::DeviceRadixSort::SortPairs(S.tmp, tmp_bytes, S.key[cur], S.key[cur ^ 1], S.perm[cur],
-                                                     S.perm[cur ^ 1], (int)n, 0, 32 + nbits, st));
+                                                     S.perm[cur ^ 1], (int)n, 0, 32 + level, st));
         cur ^= 1;
         c->launches += 3;
     }
