@@ -20,8 +20,9 @@
  *
  * Conventions
  *   - SI units: metres, coulombs, C/m^2, V/m, V.   k_e = 1/(4 pi eps0), eps0 = 8.8541878128e-12 F/m.
- *   - All arithmetic on the device is fp32 (two-level fp32 accumulation, fp64 only in the O(N) pack
- *     and fix-up steps).  Every step of the path runs in the library's CUDA kernels.
+ *   - The interactions are computed in fp32 and summed in fp32 over one block of 256 sources (34 panels); the
+ *     block sums are accumulated in fp64.  Results are fp32.  Every step of the path runs in
+ *     the library's CUDA kernels.
  *   - Pointers named d_* are DEVICE pointers owned by the caller (e.g. torch tensors), 16-byte
  *     aligned; pointers named h_* are HOST pointers.  The library copies / repacks on set_* into
  *     buffers it owns: an input may be freed or overwritten as soon as the stream has passed the

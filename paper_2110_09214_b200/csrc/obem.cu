@@ -6,7 +6,7 @@
  * Design (DESIGN.md has the long form):
  *   - Both sums are "point source -> target" sums with the same body; a panel is 7 point sources
  *     (7-point degree-5 rule, reading A1) derived once per geometry in fp64 (pack_panels_kernel).
- *   - One persistent kernel (obem_eval_kernel) covers charges AND panel sources in one launch.
+ *   - One persistent kernel per source section (obem_eval_kernel: charges, obem_panels_kernel: panels).
  *     Work is the linearised space (target tile, source block); every CTA gets an equal contiguous
  *     share of it ("stream-K" split), so there is no wave-quantisation tail at any problem size.
  *     Tiles a CTA covers completely are written directly; tiles split between CTAs go through a
@@ -14,9 +14,12 @@
  *   - Inner loop: 8 targets per thread held as 4 packed f32x2 register pairs; each source is one
  *     broadcast LDS.128 from a shared-memory ring that a single thread fills with 1-D TMA bulk
  *     copies (cp.async.bulk + mbarrier); arithmetic is Blackwell's packed FADD2/FMUL2/FFMA2
- *     (13 per target pair and source) + 2 MUFU.RSQ -- half the issue slots of scalar code at the
- *     same FP32 lane throughput.
- *   - fp32 accumulation is two-level: per 256-source block, then flushed into a running sum.
+ *     (12 per target pair and source in a block of one weight, 13 otherwise) + 2 MUFU.RSQ -- half
+ *     the issue slots of scalar code at the same FP32 lane throughput.
+ *   - The charges are kept in CLASS ORDER (stably sorted by q at obem_set_charges), so every block is of
+ *     one weight whatever order the caller stores electrons and ions in; results are scattered back.
+ *   - Accumulation: fp32 inside one block (phi as 4 short chains of 4-term trees), then fp64 running
+ *     sums in shared memory; split tiles are exchanged and summed in fp64.
  *   - No tensor cores: the path is not a dense contraction.  No CPU fallback anywhere.
  *
  * This file shares no code, header, table or constant with oracle/.
@@ -46,7 +49,7 @@ namespace {
 #define OBEM_UNR 4
 #endif
 #ifndef OBEM_DEPTH
-#define OBEM_DEPTH 3 /* re-swept after the per-section split: 1..8 -> 418.1 415.0 412.7 420.5 413.1 413.1 - 413.1 ms (N-body, config 3) */
+#define OBEM_DEPTH 3 /* pipeline distance of the general (non-uniform) point loop; the uniform loops have their own knobs */
 #endif
 #ifndef OBEM_PHI_PARTS
 #define OBEM_PHI_PARTS 4 /* separate fp32 phi chains per uniform 256-source block */
