@@ -204,3 +204,62 @@ def test_reserve_after_set_discards_the_sets(torch_cuda, api, ctx):
     ctx.set_panels(dev(torch, wl.verts), dev(torch, wl.sigma))
     ctx.set_charges(dev(torch, wl.xyzq))
     assert torch.equal(ctx.eval_at_charges(), a)
+
+
+def test_pair_order_config3_nn_sampled_tiles(torch_cuda, api, ctx, ref):
+    """The NN approximation on config 3's charges in pair-creation order: the k-d order is the
+    library's own, so the caller's order only changes which rows the results land in.  Four sampled tiles against the
+    NN oracle (identical near / far decisions: same unit count) at the path's tolerance."""
+    from oracle import nn
+    torch = torch_cuda
+    wl = W.pair_creation_order(W.make_workload(3, mesh_div=8))
+    ctx.set_softening(wl.eps_pp, 0.0)
+    ctx.set_nn_theta(2.0)
+    ctx.set_charges(dev(torch, wl.xyzq))
+    got = ctx.eval_at_charges_nn(flags=api.NBODY)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    assert np.isfinite(got).all()
+    units = ctx.nn_last_units()
+    groups = np.sort(np.random.default_rng([61, 33]).choice(wl.n_charges // 2048, 4, replace=False))
+    exp, tree = nn.nn_field(wl.xyzq, wl.eps_pp, 2.0, groups=groups, ref=ref)
+    idx = np.nonzero(np.isfinite(exp[:, 0]))[0]
+    assert idx.size == 4 * 2048
+    assert_parity(got[idx], exp[idx], "cfg3 pair order, nn, sampled tiles")
+    assert units == nn.units(tree, 2.0, wl.n_charges)
+
+
+def test_e_only_is_bit_identical_in_E_and_zero_in_phi(torch_cuda, api, ctx, ref):
+    """OBEM_NO_PHI (Eq 3.8 and 2.14 are field sums; the integrators read only E): E of the
+    E-only instantiations equals E of the E + phi ones bit for bit, the phi lane is 0 -- at the charges (big tiles,
+    pair order, split tiles), on a sub-range, at free points, and for a tiny problem (small-tile instantiations).  Not
+    with the exact near-field correction or the partner by-product."""
+    torch = torch_cuda
+    wl = W.pair_creation_order(W.make_workload(2, charge_div=4, mesh_div=2))       # 16384 charges, 4096 panels
+    tiny = W.make_workload(1)
+    for w in (wl, tiny):
+        ctx.set_softening(w.eps_pp, w.eps_panel)
+        ctx.set_panels(dev(torch, w.verts), dev(torch, w.sigma))
+        ctx.set_charges(dev(torch, w.xyzq))
+        for flags in (api.NBODY, api.PANELS, api.NBODY | api.PANELS):
+            full = ctx.eval_at_charges(flags=flags)
+            eo = ctx.eval_at_charges(flags=flags | api.NO_PHI)
+            assert torch.equal(eo[:, :3], full[:, :3]), "E differs, flags %d" % flags
+            assert torch.all(eo[:, 3] == 0)
+        part = ctx.eval_at_charges_range(1000, 2500, flags=api.NBODY | api.PANELS)
+        part_eo = ctx.eval_at_charges_range(1000, 2500, flags=api.NBODY | api.PANELS | api.NO_PHI)
+        assert torch.equal(part_eo[:, :3], part[:, :3]) and torch.all(part_eo[:, 3] == 0)
+        pts = dev(torch, w.xyzq[:3000] + np.float32(0.2 * UM))
+        a = ctx.eval_at_points(pts, flags=api.NBODY | api.PANELS)
+        b = ctx.eval_at_points(pts, flags=api.NBODY | api.PANELS | api.NO_PHI)
+        assert torch.equal(b[:, :3], a[:, :3]) and torch.all(b[:, 3] == 0)
+    on, op = ref.eval_field(xyzq=tiny.xyzq, verts=tiny.verts, sigma=tiny.sigma, eps_pp=tiny.eps_pp)
+    eo = ctx.eval_at_charges(flags=api.NBODY | api.PANELS | api.NO_PHI).cpu().numpy().astype(np.float64)
+    dE = np.linalg.norm(eo[:, :3] - (on + op)[:, :3], axis=1)
+    assert np.sqrt((dE ** 2).sum() / (np.linalg.norm((on + op)[:, :3], axis=1) ** 2).sum()) <= 2e-5
+    with pytest.raises(api.ObemError) as e:
+        ctx.eval_at_charges(flags=api.PANELS | api.PANELS_EXACT | api.NO_PHI)
+    assert e.value.status == -1
+    with pytest.raises(api.ObemError) as e:
+        ctx.eval_at_charges_partners(flags=api.NBODY | api.NO_PHI)
+    assert e.value.status == -1
