@@ -23,6 +23,7 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared",  # cudart is linked statically (nvcc default): no search-path dependency
+    "--threads", "0",                  # the translation units compile in parallel
 ]
 
 
