@@ -36,7 +36,10 @@ constexpr int M_TT = M_THREADS * 2 * M_NP;   /* targets per tile                
 constexpr int M_STAGES = 4;
 constexpr int M_KS = 4;                      /* density vectors per pass                        */
 constexpr int M_SROW = 36;                   /* floats per (block, vector) sigma row: PPB = 34 padded to 144 B */
-constexpr int M_DEPTH = 4;                   /* software-pipeline distance of the source loop   */
+#ifndef OBEM_M_DEPTH
+#define OBEM_M_DEPTH 4
+#endif
+constexpr int M_DEPTH = OBEM_M_DEPTH;        /* software-pipeline distance of the source loop   */
 constexpr double M_KE = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12); /* reading A7 */
 
 struct MultiParams {
