@@ -443,6 +443,36 @@ def run_ours(args):
         ctx.set_charges(d_x)
         del d_xp
 
+    # ---- small configs are launch-latency-bound: the same step replayed from a CUDA graph (no launch gaps) ----
+    if world == 1 and n <= 131072:
+        side = torch.cuda.Stream()
+        side.wait_stream(stream)
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            ctx.set_panels(d_verts, d_sigma, stream=side)          # sizes every library-owned buffer before capture
+            ctx.set_charges(d_x, stream=side)
+            ctx.eval_at_charges_range(first, count, out=out, flags=api.NBODY | api.PANELS, stream=side)
+            side.synchronize()
+            with torch.cuda.graph(graph, stream=side):
+                ctx.set_panels(d_verts, d_sigma, stream=side)
+                ctx.set_charges(d_x, stream=side)
+                ctx.eval_at_charges_range(first, count, out=out, flags=api.NBODY | api.PANELS, stream=side)
+        torch.cuda.synchronize()
+        reps = 50
+        graph.replay()
+        torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record(stream)
+        for _ in range(reps):
+            graph.replay()
+        b.record(stream)
+        torch.cuda.synchronize()
+        g_ms = a.elapsed_time(b) / reps
+        extras["step_cuda_graph"] = {"ms_per_step": g_ms, "Ginteractions_per_s": total_inter / (g_ms * 1e-3) / 1e9,
+                                     "what": "the same step (set_panels + set_charges + evaluation) captured once in a "
+                                             "CUDA graph and replayed %d times back to back, L2 warm: what is left "
+                                             "when the launch gaps are gone" % reps}
+
     # ---- supplementary, N = 1 only: the adjacent steps, each against its own roofline ----
     if world == 1 and not args.no_next:
         extras["next1"] = bench_next1(torch, api, ctx, wl, timed, dev, extras["panels_only"]["s"])
