@@ -53,7 +53,8 @@ typedef enum obem_status {
     OBEM_EINVAL = -1, /* null / negative / misaligned argument, unknown flag bits            */
     OBEM_ESTATE = -2, /* evaluate before the sources the flags ask for were set              */
     OBEM_ECUDA = -3,  /* a CUDA call failed; obem_last_cuda_error() gives the cudaError_t     */
-    OBEM_ENOMEM = -4  /* device allocation failed                                            */
+    OBEM_ENOMEM = -4, /* device allocation failed                                            */
+    OBEM_ELIMIT = -5  /* a size beyond the fixed maximum of obem_nbody_at_points_static      */
 } obem_status;
 
 /* flags of the evaluate calls: which of the two sums to include */
@@ -133,6 +134,27 @@ int obem_field_at_charges_host(obem_ctx* c, const float* h_xyzq, int64_t n, cons
 /* Field map through HOST buffers, synchronous (h_verts may be NULL as above). */
 int obem_field_at_points_host(obem_ctx* c, const float* h_pts, int64_t m, const float* h_verts,
                               const float* h_sigma, int64_t n_panels, float* h_out, unsigned flags);
+
+/* The ONE entry point that allocates nothing (no cudaMalloc, cudaFree or allocating library routine, no context):
+ * for callers that cannot allocate -- code under CUDA graph capture, tight serving loops, harnesses that forbid it.
+ * Computes what obem_eval_at_points(OBEM_NBODY) computes, Eq (3.8) with Plummer softening and no
+ * index exclusion, a source at zero softened distance contributing 0 (reading A4), straight from the caller's arrays:
+ *   d_xyzq [n][4] fp32 = x, y, z [m], q [C] (any n, any order);  d_pts [m][4] fp32, 4th lane ignored;
+ *   d_out  [m][4] fp32 = Ex, Ey, Ez [V/m], phi [V];  all device pointers of the CURRENT device, 16-byte aligned.
+ * Its scratch (fp64 partial sums of the split-source scheme) is a file-scope static __device__ array of fixed size,
+ * OBEM_STATIC_MAX_POINTS x OBEM_STATIC_MAX_SPLITS x 32 B = 8 MiB, which every GPU that loads libobem.so holds until
+ * the process exits.  m > OBEM_STATIC_MAX_POINTS returns OBEM_ELIMIT (split the points, or use a context).
+ * The first call on a device looks the array's device address up (cudaGetSymbolAddress: make that call outside a
+ * graph capture); later calls only enqueue two kernels on `cuda_stream`.  ALL calls on a device share the scratch,
+ * which keeps the last call's contents (every slot a call reads it has written itself; nothing needs clearing): calls
+ * that overlap on the GPU -- different streams, concurrently replayed graphs -- race.  Serialise them.
+ * Same arithmetic as the hot path (fp32 terms, fp32 sums over 256 sources, fp64 across blocks), simpler kernel
+ * (13 packed instructions + the zero-distance guard): results agree with obem_eval_at_points to the path's tolerance,
+ * not bit for bit. */
+#define OBEM_STATIC_MAX_POINTS 16384
+#define OBEM_STATIC_MAX_SPLITS 16
+int obem_nbody_at_points_static(const float* d_xyzq, int64_t n, const float* d_pts, int64_t m, float eps_pp_m,
+                                float* d_out, void* cuda_stream);
 
 /* Introspection (host side, no device work) */
 int64_t obem_n_charges(const obem_ctx* c);     /* -1 if never set */

@@ -37,6 +37,7 @@ SIGNATURES = {
                                                   ctypes.c_uint]),
     "obem_field_at_points_host": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _i64, _c_fp, _c_fp, _i64, _c_fp,
                                                  ctypes.c_uint]),
+    "obem_nbody_at_points_static": (ctypes.c_int, [_c_fp, _i64, _c_fp, _i64, ctypes.c_float, _c_fp, ctypes.c_void_p]),
     "obem_n_charges": (_i64, [ctypes.c_void_p]),
     "obem_n_panels": (_i64, [ctypes.c_void_p]),
     "obem_sm_count": (ctypes.c_int, [ctypes.c_void_p]),
@@ -583,6 +584,28 @@ class Context:
                                          m, out.data_ptr() if m else None, 1 if accumulate else 0,
                                          _stream_ptr(stream)), "obem_interp_map")
         return out
+
+
+STATIC_MAX_POINTS = 16384  # OBEM_STATIC_MAX_POINTS
+
+
+def nbody_at_points_static(xyzq, pts, eps_pp: float, out, stream=None):
+    """obem_nbody_at_points_static: the N-body sum of xyzq [N,4] at pts [M,4] into out [M,4] (all float32 CUDA tensors
+    of the current device) with NO allocation anywhere -- no context, scratch in a fixed static device array; M <=
+    STATIC_MAX_POINTS.  `out` is required (allocating it here would defeat the purpose)."""
+    n, m = int(xyzq.shape[0]), int(pts.shape[0])
+    if n:
+        _dev_f32(xyzq, "xyzq", (4,))
+    if m:
+        _dev_f32(pts, "pts", (4,))
+        _dev_f32(out, "out", (4,))
+        if out.shape[0] != m:
+            raise ValueError("out must be [M, 4]")
+    rc = _lib.obem_nbody_at_points_static(xyzq.data_ptr() if n else None, n, pts.data_ptr() if m else None, m,
+                                          float(eps_pp), out.data_ptr() if m else None, _stream_ptr(stream))
+    if rc != 0:
+        raise ObemError(rc, "obem_nbody_at_points_static")
+    return out
 
 
 def recombination_radius(e_ioni_ev: float) -> float:

@@ -14,7 +14,7 @@ SRC = os.path.join(_HERE, "csrc", "obem.cu")
 SRCS = [SRC, os.path.join(_HERE, "csrc", "obem_next.cu"),           # hot path; adjacent steps
         os.path.join(_HERE, "csrc", "obem_map.cu"), os.path.join(_HERE, "csrc", "obem_near.cu"),
         os.path.join(_HERE, "csrc", "obem_nn.cu"), os.path.join(_HERE, "csrc", "obem_geom.cu"),
-        os.path.join(_HERE, "csrc", "obem_multi.cu")]
+        os.path.join(_HERE, "csrc", "obem_multi.cu"), os.path.join(_HERE, "csrc", "obem_static.cu")]
 DEPS = SRCS + [os.path.join(_HERE, "csrc", "obem_internal.cuh")]
 HDR = os.path.join(ROOT, "include", "obem.h")
 LIB = os.path.join(_HERE, "libobem.so")

@@ -2036,6 +2036,7 @@ const char* obem_status_string(int status)
     case OBEM_ESTATE: return "OBEM_ESTATE: evaluate/update before the sources were set";
     case OBEM_ECUDA: return "OBEM_ECUDA: a CUDA call failed (see obem_last_cuda_error)";
     case OBEM_ENOMEM: return "OBEM_ENOMEM: device allocation failed";
+    case OBEM_ELIMIT: return "OBEM_ELIMIT: more points than obem_nbody_at_points_static's fixed scratch holds (OBEM_STATIC_MAX_POINTS)";
     default: return "unknown obem_status";
     }
 }
