@@ -317,7 +317,8 @@ template <bool TRACK, bool PHI, int NS, int NPAIR>
 __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2,
                                                    const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
-                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[2 * NPAIR])
+                                                   u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[2 * NPAIR],
+                                                   const int jb = 0, const int je = NS)
 {
     constexpr Knobs KN = TRACK ? KNOBS_T : (PHI ? KNOBS_PHI : KNOBS_E);
     constexpr int DEPTH = KN.d;
@@ -325,7 +326,7 @@ __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s,
     constexpr int K = UNR * NPAIR;
     static_assert(UNR == 4, "the phi tree below sums the 4 sources of a trip");
 #pragma unroll 1
-    for (int j0 = 0; j0 < NS; j0 += UNR) {
+    for (int j0 = jb; j0 < je; j0 += UNR) { /* [jb, je): the whole NS sources unless the caller says otherwise */
         float4 q[UNR];
 #pragma unroll
         for (int j = 0; j < UNR; ++j) q[j] = s[j0 + j];
@@ -762,6 +763,27 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
                     self_block_loop<TRACK, PHI, NSP, NPAIR>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0],
                                                      rel, h * NSP, bm, negmask, posmask);
                 phi_join();
+            } else if (LIST && !(blkw == blkw) && ring[st][0].z > 0.f) {
+                /* NN leaf of -|w| and +|w| members, negatives first (nn_leaf_kernel): the two runs are summed
+                 * unweighted by the 12-instruction loop, negatives into a second accumulator set; then
+                 * a = |w| (a - b), and the one 4-source group that straddles the sign boundary goes through the
+                 * general loop with its true weights */
+                const float wmag = ring[st][0].z;
+                const int n4 = (int)ring[st][0].w & ~3;
+                u64 bX[NPAIR], bY[NPAIR], bZ[NPAIR], bP[NPAIR];
+#pragma unroll
+                for (int p = 0; p < NPAIR; ++p) bX[p] = bY[p] = bZ[p] = bP[p] = 0ull;
+                block_loop_uniform<false, PHI, SB, NPAIR>(sblk, eps2, X, Y, Z, bX, bY, bZ, bP, bm, 0, n4);
+                block_loop_uniform<false, PHI, SB, NPAIR>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, bm, n4 + 4 < SB ? n4 + 4 : SB, SB);
+                const u64 w2 = pk(wmag, wmag);
+#pragma unroll
+                for (int p = 0; p < NPAIR; ++p) {
+                    aX[p] = mul2(sub2(aX[p], bX[p]), w2);
+                    aY[p] = mul2(sub2(aY[p], bY[p]), w2);
+                    aZ[p] = mul2(sub2(aZ[p], bZ[p]), w2);
+                    if (PHI) aP[p] = mul2(sub2(aP[p], bP[p]), w2);
+                }
+                if (n4 < SB) block_loop<false, PHI, 4, NPAIR>(sblk + n4, eps2, X, Y, Z, aX, aY, aZ, aP, bm);
             } else if (blkw == blkw) {
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)

@@ -174,22 +174,51 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
     keys[i] = ((u64k)rank << 32) | (u64k)low; /* `level` bits of segment rank + 32 of coordinate: 4-6 radix passes */
 }
 
-/* one CTA per leaf: sorted copy (plain, padded) + blocked copy with header + bounding box + the two pseudo-particles */
+/* one CTA per leaf: sorted copy (plain, padded) + blocked copy with header + bounding box + the two pseudo-particles.
+ * Inside the leaf the members are put in the order negative weights first (a stable partition: which charges a leaf
+ * holds is the k-d order's business, their order inside it enters no result), and perm_out records the final order.
+ * Header: .x = the weight all 256 members share, or NaN; .z = |w| if the leaf is full and its members carry exactly
+ * -|w| and +|w| (electrons and singly charged ions: the usual leaf), else 0; .w = the number of negative members.
+ * The list kernel then sums the negative and the positive run unweighted (12 packed instructions per interaction
+ * instead of 13) and only the 4-source group that straddles the sign boundary with weights. */
 __global__ void __launch_bounds__(LEAF) nn_leaf_kernel(const float4* __restrict__ x, const int* __restrict__ perm,
                                                         long long n, float4* __restrict__ sorted,
                                                         float4* __restrict__ pool, float* __restrict__ leafbox,
-                                                        float4* __restrict__ pseudo, double* __restrict__ leafmom)
+                                                        float4* __restrict__ pseudo, double* __restrict__ leafmom,
+                                                        int* __restrict__ perm_out)
 {
     __shared__ double red[8][LEAF / 32];
     __shared__ float fred[6][LEAF / 32];
+    __shared__ int wneg[LEAF / 32];
     const long long l = blockIdx.x, i = l * LEAF + threadIdx.x;
     const bool valid = i < n;
-    const float4 v = valid ? x[perm[i]] : make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
-    sorted[i] = v;
-    pool[l * OBEM_SBH + 1 + threadIdx.x] = v;
-    const float w0 = x[perm[l * LEAF]].w;
-    const int uniform = __syncthreads_and(v.w == w0);
-    if (threadIdx.x == 0) pool[l * OBEM_SBH] = make_float4(uniform ? w0 : __int_as_float(0x7fc00000), 0.f, 0.f, 0.f);
+    const int src = valid ? perm[i] : -1;
+    const float4 v = valid ? x[src] : make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
+    /* stable partition: negatives first */
+    const bool neg = valid && v.w < 0.f;
+    {
+        const unsigned bal = __ballot_sync(0xffffffffu, neg);
+        if ((threadIdx.x & 31) == 0) wneg[threadIdx.x >> 5] = __popc(bal);
+        __syncthreads();
+        int before = 0, total = 0;
+        for (int ww = 0; ww < LEAF / 32; ++ww) {
+            if (ww < (int)(threadIdx.x >> 5)) before += wneg[ww];
+            total += wneg[ww];
+        }
+        const int in_warp = __popc(bal & ((1u << (threadIdx.x & 31)) - 1u));
+        const int rank_neg = before + in_warp;
+        const int slot = neg ? rank_neg : total + ((int)threadIdx.x - rank_neg);
+        const long long j = l * LEAF + slot;
+        sorted[j] = v;
+        pool[l * OBEM_SBH + 1 + slot] = v;
+        if (j < n) perm_out[j] = src; /* invalid members are the last threads of the last leaf: they stay last */
+        const float w0 = x[perm[l * LEAF]].w, m0 = fabsf(w0);
+        const int uniform = __syncthreads_and(v.w == w0);
+        const int twoval = __syncthreads_and(valid && m0 > 0.f && fabsf(v.w) == m0);
+        if (threadIdx.x == 0)
+            pool[l * OBEM_SBH] = make_float4(uniform ? w0 : __int_as_float(0x7fc00000), 0.f,
+                                             (twoval && !uniform) ? m0 : 0.f, (float)total);
+    }
     /* box over the valid members, charge and first moment of the positive and of the negative members */
     const float big = __int_as_float(0x7f800000);
     float lo[3] = {valid ? v.x : big, valid ? v.y : big, valid ? v.z : big};
@@ -519,7 +548,8 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     const int* perm = S.perm[cur];
     /* 2. leaves */
     nn_leaf_kernel<<<(unsigned)n_leaf, LEAF, 0, st>>>(c->d_chg, perm, n, S.sorted, S.pool, S.leafbox, S.pseudo,
-                                                      S.leafmom);
+                                                      S.leafmom, S.perm[cur ^ 1]);
+    perm = S.perm[cur ^ 1]; /* the k-d order with the sign partition inside the leaves */
     OBEM_CUDA(c, cudaGetLastError());
     nn_super_kernel<<<(unsigned)ceil_div(n_super, 64), 64, 0, st>>>(S.leafbox, S.leafmom, n_leaf, n_super, S.superbox,
                                                                     S.superpseudo);
