@@ -244,6 +244,12 @@ struct obem_ctx {
     float4* d_exact_tmp = nullptr;    /* [nt] panel part of an N-body + exact-panels evaluation */
     long long exact_tmp_cap = 0;
     long long near_entries = -1; /* (cell, panel) entries of the current lists; -1 before the first build */
+    /* the targets of one evaluation grouped by cell (near_tcount / near_tfill) */
+    int* d_near_tcell = nullptr;  /* [nt] cell of every target, -1 = none */
+    int* d_near_tlist = nullptr;  /* [nt] targets in cell order */
+    int* d_near_tcount = nullptr; /* [ncells + 1] targets per cell; then the fill cursor */
+    int* d_near_tstart = nullptr; /* [ncells + 1] its exclusive scan; [ncells] = targets that have a cell */
+    long long near_t_cap = 0, near_c_cap = 0;
     obem_nn_state nn;
     /* obem_geom.cu: symmetry planes and polygonal cells */
     int sym_n = 0, sym_axis[3] = {0, 0, 0}, sym_sign[3] = {1, 1, 1};

@@ -193,9 +193,12 @@ __device__ void tri_exact(const double (&v)[3][3], const double (&r)[3], double&
     const double d = nx * (r[0] - v[0][0]) + ny * (r[1] - v[0][1]) + nz * (r[2] - v[0][2]);
     const double ad = fabs(d);
     double sb = 0.0;
-#pragma unroll
+    /* NOT unrolled, and one log call site: the fp64 log / atan routines are inlined wherever they are called, and
+     * with three copies of the edge body the correction kernel spent most of its issue slots waiting for instructions
+     * (ncu: stall "no instruction" 15.9 per issue) */
+#pragma unroll 1
     for (int i = 0; i < 3; ++i) {
-        const int i1 = (i + 1) % 3;
+        const int i1 = (i == 2) ? 0 : i + 1;
         /* vectors from r to the two ends of the edge; their in-plane parts are (a - rho), (b - rho) */
         const double ax = v[i][0] - r[0], ay = v[i][1] - r[1], az = v[i][2] - r[2];
         const double bx = v[i1][0] - r[0], by = v[i1][1] - r[1], bz = v[i1][2] - r[2];
@@ -209,17 +212,16 @@ __device__ void tri_exact(const double (&v)[3][3], const double (&r)[3], double&
         const double lm = ax * lx + ay * ly + az * lz, lp = bx * lx + by * ly + bz * lz;
         const double Rm = sqrt(ax * ax + ay * ay + az * az), Rp = sqrt(bx * bx + by * by + bz * bz);
         const double R02 = P0 * P0 + d * d;
-        double f;
+        double num, den; /* the same three forms as before, the operands selected first */
         if (lm >= 0.0) {
-            if (!(Rm + lm > 0.0)) continue;
-            f = log((Rp + lp) / (Rm + lm));
+            num = Rp + lp, den = Rm + lm;
         } else if (lp <= 0.0) {
-            if (!(Rp - lp > 0.0)) continue;
-            f = log((Rm - lm) / (Rp - lp));
+            num = Rm - lm, den = Rp - lp;
         } else {
-            if (!(R02 > 0.0)) continue;
-            f = log((Rp + lp) * (Rm - lm) / R02);
+            num = (Rp + lp) * (Rm - lm), den = R02;
         }
+        if (!(den > 0.0)) continue;
+        const double f = log(num / den);
         double beta = 0.0;
         if (P0 != 0.0) beta = atan(P0 * lp / (R02 + ad * Rp)) - atan(P0 * lm / (R02 + ad * Rm));
         I_phi += P0 * f - ad * beta;
@@ -267,7 +269,7 @@ __device__ __forceinline__ bool near_pair(const NearParams& P, int p, const floa
     const float4 o = __ldg(P.porg + p);
     const double TX = (double)__fsub_rn(t.x, o.x), TY = (double)__fsub_rn(t.y, o.y), TZ = (double)__fsub_rn(t.z, o.z);
     double r2min = 1e300;
-#pragma unroll
+#pragma unroll 1
     for (int k = 0; k < 7; ++k) {
         const float4 q = __ldg(P.qrel + (long long)p * 7 + k);
         const double dx = TX - (double)q.x, dy = TY - (double)q.y, dz = TZ - (double)q.z;
@@ -290,23 +292,73 @@ __device__ __forceinline__ bool near_pair(const NearParams& P, int p, const floa
     return r2min < P.crit2 * R * R;
 }
 
-constexpr int NEAR_WARPS = 2; /* small CTAs: most warps leave at once (no near panel): 14.5 -> 12.3 ms on config 3 against 8 warps */
+#ifndef OBEM_NEAR_WARPS
+#define OBEM_NEAR_WARPS 2
+#endif
+#ifndef OBEM_NEAR_MINB
+#define OBEM_NEAR_MINB 24
+#endif
+constexpr int NEAR_WARPS = OBEM_NEAR_WARPS; /* small CTAs: most warps leave at once (no near panel): 14.5 -> 12.3 ms on config 3 against 8 warps */
 /* A target closer than VERY_NEAR * h_p to a quadrature source of panel p: that one 7-point term exceeds the whole
  * local field by more than 0.013 / VERY_NEAR^2 (= 13 at 1/32), and what it cost the fp32 accumulation of the
  * evaluation kernel (an ulp of ITS size) cannot be corrected afterwards.  Such targets are recomputed from scratch
  * in fp64 by near_redo_kernel. */
 constexpr double VERY_NEAR = 1.0 / 32.0;
 
+/* cell of a target, -1 if it lies outside the grid (no near panel can exist; also NaN) */
+__device__ __forceinline__ long long near_cell_of(const NearGrid& g, const float4 t)
+{
+    const double tq[3] = {(double)t.x, (double)t.y, (double)t.z};
+    int ci[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const double u = floor((tq[a] - g.lo[a]) * g.inv_s);
+        if (!(u >= 0.0 && u < (double)g.n[a])) return -1;
+        ci[a] = (int)u;
+    }
+    return ((long long)ci[0] * g.n[1] + ci[1]) * g.n[2] + ci[2];
+}
+/* cell of every target (-1: none, or an empty cell) and the number of targets per cell */
+__global__ void __launch_bounds__(256) near_tcount_kernel(const NearParams P, int* __restrict__ tcell, int* __restrict__ tcount)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.nt) return;
+    long long cell = near_cell_of(P.g, P.tgt[i]);
+    if (cell >= 0 && P.start[cell] == P.start[cell + 1]) cell = -1;
+    tcell[i] = (int)cell;
+    if (cell >= 0) atomicAdd(tcount + cell, 1);
+}
+/* the targets grouped by cell (any order inside a cell: it enters no result) */
+__global__ void __launch_bounds__(256) near_tfill_kernel(const int* __restrict__ tcell, const int* __restrict__ tstart,
+                                                        int* __restrict__ cursor, int* __restrict__ tlist, long long nt)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nt) return;
+    const int cell = tcell[i];
+    if (cell >= 0) tlist[tstart[cell] + atomicAdd(cursor + cell, 1)] = (int)i;
+}
+
 /* one warp per target: the lanes test 32 candidates of the target's cell at a time; the near ones are compacted
  * into a per-warp queue so that the expensive closed form always runs on full warps */
-/* latency-bound (dependent fp64 log / atan chains, per-pair loads): more resident warps beat fewer spills -- A/B on config 3
- * with the register cap of 2..32 CTAs/SM: 12.4 (108 registers), 11.0 (96), 10.1 (72), 8.8 (48), 8.1 (40), 8.6 (32) ms */
-__global__ void __launch_bounds__(NEAR_WARPS * 32, 24) near_correct_kernel(const NearParams P)
+/* Round 1: latency-bound (dependent fp64 log / atan chains, per-pair loads): more resident warps beat fewer spills --
+ * A/B on config 3 with the register cap of 2..32 CTAs/SM: 12.4 (108 registers), 11.0 (96), 10.1 (72), 8.8 (48), 8.1 (40),
+ * 8.6 (32) ms.  Round 2 (config 3): 8.05 ms -> 5.4 with the targets in cell order (panel records hit L1) -> 3.45 with the
+ * edge loop of tri_exact rolled and one log call site -> 3.03 with the 7-point loop rolled too (the kernel was waiting
+ * for INSTRUCTIONS: 14,000 SASS lines of inlined fp64 log / atan / sqrt copies; now 5,000); warps per CTA and the
+ * register cap no longer matter (3.0 .. 3.3 ms over 1..8 warps, 4..32 CTAs/SM). */
+/* Round 2: the warps take the targets in CELL order (order[], from near_tcount / near_tfill below), not in the
+ * caller's order: the warps that are resident together then walk the same cell's panel list and read the same panel
+ * records, so those loads hit L1 instead of going to L2 one by one; and the targets that have no cell (3 of 4 in
+ * config 3) never get a warp.  Which warp handles a target enters no result: each target still sums its own panels
+ * in ascending order, alone. */
+__global__ void __launch_bounds__(NEAR_WARPS * 32, OBEM_NEAR_MINB) near_correct_kernel(const NearParams P, const int* __restrict__ order,
+                                                                          const int* __restrict__ n_order)
 {
     __shared__ int queue[NEAR_WARPS][64];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const long long t_idx = (long long)blockIdx.x * NEAR_WARPS + w;
-    if (t_idx >= P.nt) return;
+    const long long slot = (long long)blockIdx.x * NEAR_WARPS + w;
+    if (slot >= (long long)*n_order) return;
+    const long long t_idx = order[slot];
     const float4 t = P.tgt[t_idx];
     int ci[3];
     const double tq[3] = {(double)t.x, (double)t.y, (double)t.z};
@@ -587,7 +639,45 @@ int obem_near_correct(obem_ctx* c, const float4* tgt, long long nt, float4* out,
     P.eps2 = (double)c->eps_panel * (double)c->eps_panel;
     P.crit2 = (VERY_NEAR / (double)c->near_factor) * (VERY_NEAR / (double)c->near_factor);
     P.redo_list = c->d_redo_list, P.redo_count = c->d_redo_count;
-    near_correct_kernel<<<(unsigned)ceil_div(nt, NEAR_WARPS), NEAR_WARPS * 32, 0, st>>>(P);
+    /* the targets in cell order: count, scan, fill (three O(nt) passes) */
+    const long long ncells = (long long)c->near_n[0] * c->near_n[1] * c->near_n[2];
+    if (nt > c->near_t_cap) {
+        if (c->d_near_tcell) cudaFree(c->d_near_tcell);
+        if (c->d_near_tlist) cudaFree(c->d_near_tlist);
+        c->d_near_tcell = c->d_near_tlist = nullptr, c->near_t_cap = 0;
+        OBEM_CUDA(c, cudaMalloc(&c->d_near_tcell, (size_t)nt * sizeof(int)));
+        OBEM_CUDA(c, cudaMalloc(&c->d_near_tlist, (size_t)nt * sizeof(int)));
+        c->near_t_cap = nt;
+    }
+    if (ncells + 1 > c->near_c_cap) {
+        if (c->d_near_tcount) cudaFree(c->d_near_tcount);
+        if (c->d_near_tstart) cudaFree(c->d_near_tstart);
+        c->d_near_tcount = c->d_near_tstart = nullptr, c->near_c_cap = 0;
+        OBEM_CUDA(c, cudaMalloc(&c->d_near_tcount, (size_t)(ncells + 1) * sizeof(int)));
+        OBEM_CUDA(c, cudaMalloc(&c->d_near_tstart, (size_t)(ncells + 1) * sizeof(int)));
+        c->near_c_cap = ncells + 1;
+    }
+    size_t tmp = 0;
+    OBEM_CUDA(c, cub::DeviceScan::ExclusiveSum(nullptr, tmp, c->d_near_tcount, c->d_near_tstart, (int)(ncells + 1), st));
+    if (tmp > c->scan_tmp_cap) {
+        if (c->d_scan_tmp) cudaFree(c->d_scan_tmp);
+        c->d_scan_tmp = nullptr, c->scan_tmp_cap = 0;
+        OBEM_CUDA(c, cudaMalloc(&c->d_scan_tmp, tmp));
+        c->scan_tmp_cap = tmp;
+    }
+    OBEM_CUDA(c, cudaMemsetAsync(c->d_near_tcount, 0, (size_t)(ncells + 1) * sizeof(int), st));
+    near_tcount_kernel<<<(unsigned)ceil_div(nt, 256), 256, 0, st>>>(P, c->d_near_tcell, c->d_near_tcount);
+    OBEM_CUDA(c, cudaGetLastError());
+    tmp = c->scan_tmp_cap;
+    OBEM_CUDA(c, cub::DeviceScan::ExclusiveSum(c->d_scan_tmp, tmp, c->d_near_tcount, c->d_near_tstart, (int)(ncells + 1), st));
+    OBEM_CUDA(c, cudaMemsetAsync(c->d_near_tcount, 0, (size_t)(ncells + 1) * sizeof(int), st)); /* now the fill cursor */
+    near_tfill_kernel<<<(unsigned)ceil_div(nt, 256), 256, 0, st>>>(c->d_near_tcell, c->d_near_tstart, c->d_near_tcount,
+                                                                 c->d_near_tlist, nt);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 3;
+    /* grid for the worst case (every target has a cell); warps beyond tstart[ncells] leave at once */
+    near_correct_kernel<<<(unsigned)ceil_div(nt, NEAR_WARPS), NEAR_WARPS * 32, 0, st>>>(P, c->d_near_tlist,
+                                                                                       c->d_near_tstart + ncells);
     OBEM_CUDA(c, cudaGetLastError());
     near_redo_kernel<<<4 * c->sm_count, 256, 0, st>>>(P, c->n_pan);
     OBEM_CUDA(c, cudaGetLastError());
@@ -623,7 +713,8 @@ int obem_eval_exact(obem_ctx* c, const float4* tgt, long long nt, float4* out, u
 void obem_near_free(obem_ctx* c)
 {
     void* ptrs[] = {c->d_pverts, c->d_psigma, c->d_porg, c->d_pcr, c->d_cell_start, c->d_cell_fill, c->d_cell_list,
-                    c->d_near_red, c->d_scan_tmp, c->d_redo_list, c->d_redo_count, c->d_exact_tmp};
+                    c->d_near_red, c->d_scan_tmp, c->d_redo_list, c->d_redo_count, c->d_exact_tmp, c->d_near_tcell,
+                    c->d_near_tlist, c->d_near_tcount, c->d_near_tstart};
     for (void* p : ptrs)
         if (p) cudaFree(p);
 }
