@@ -839,12 +839,15 @@ def bench_next4(torch, api, ctx, wl, timed, dev):
 
 
 def kernel_source_hash() -> str:
-    """sha256 over the sources of the evaluation kernels: ties a recorded ncu figure to the code it was captured on."""
+    """sha256 over the sources of the evaluation kernels -- csrc/obem.cu and the device helpers of obem_internal.cuh
+    (everything before the host-side context structs): ties a recorded ncu figure to the code it was captured on."""
     import hashlib
     h = hashlib.sha256()
-    for f in ("obem.cu", "obem_internal.cuh"):
-        with open(os.path.join(ROOT, "paper_2110_09214_b200", "csrc", f), "rb") as fh:
-            h.update(fh.read())
+    base = os.path.join(ROOT, "paper_2110_09214_b200", "csrc")
+    with open(os.path.join(base, "obem.cu"), "rb") as fh:
+        h.update(fh.read())
+    with open(os.path.join(base, "obem_internal.cuh"), "rb") as fh:
+        h.update(fh.read().split(b"/* obem_nn.cu: buffers of the NN approximation")[0])
     return h.hexdigest()[:16]
 
 
