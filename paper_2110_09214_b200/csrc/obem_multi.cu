@@ -19,7 +19,7 @@
  *
  * Launch shape: persistent grid, one CTA per SM, tiles of 1024 targets (256 threads x 4) taken round-robin -- a tile
  * is never split, so there is no workspace and no fix-up; panel blocks (and the pass's sigma rows, re-blocked to
- * 36 floats per block and vector) stream through the same 4-stage TMA ring as the hot path; block sums in fp32, the
+ * 36 x 4 floats per block: the four densities of a panel side by side) stream through the same 4-stage TMA ring as the hot path; block sums in fp32, the
  * running sums in fp64 in shared memory (4 KS doubles per target).  A target at zero distance from a quadrature
  * point (reading A4) poisons its sums with inf/NaN; that is detected when the tile is written and the owning thread
  * recomputes that target in fp64 with the guard (rare: a measure-zero event).
@@ -35,6 +35,7 @@ constexpr int M_NP = 2;                      /* target pairs per thread         
 constexpr int M_TT = M_THREADS * 2 * M_NP;   /* targets per tile                                */
 constexpr int M_STAGES = 4;
 constexpr int M_KS = 4;                      /* density vectors per pass                        */
+static_assert(M_KS == 4, "the kernel reads the densities of a panel as one float4");
 constexpr int M_SROW = 36;                   /* floats per (block, vector) sigma row: PPB = 34 padded to 144 B */
 #ifndef OBEM_M_DEPTH
 #define OBEM_M_DEPTH 4
@@ -44,7 +45,7 @@ constexpr double M_KE = 1.0 / (4.0 * 3.14159265358979323846 * 8.8541878128e-12);
 
 struct MultiParams {
     const float4* unit;   /* blocked panel buffer encoded with the bare weights A_p w_k (sigma = 1)      */
-    const float* sig;     /* [nblk][ks][M_SROW] the pass's density vectors, blocked                        */
+    const float* sig;     /* [nblk][M_SROW][M_KS] the pass's density vectors, blocked                      */
     const float4* qrel;   /* [np*7] plain offsets from the frame origin, .w = A_p w_k (repair)            */
     const float* sigma;   /* [K][np] the caller's vectors (repair)                                       */
     long long np, nblk;
@@ -79,17 +80,18 @@ __global__ void __launch_bounds__(128) multi_unit_kernel(const float4* __restric
     }
 }
 
-/* sigma[k0 + s][p] -> sig[(block b, vector s, slot j)], zero beyond np and in the two pad slots */
+/* sigma[k0 + s][p] -> sig[(block b, slot j, vector s of M_KS)]: the up to 4 densities of a panel side by side, so
+ * that the kernel reads them with ONE LDS.128; zero beyond np, in the two pad slots and for vectors >= ks */
 __global__ void __launch_bounds__(256) multi_sigma_kernel(const float* __restrict__ sigma, float* __restrict__ sig,
                                                           long long np, long long nblk, int k0, int ks)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= nblk * ks * M_SROW) return;
-    const int j = (int)(i % M_SROW);
-    const long long r = i / M_SROW;
-    const int s = (int)(r % ks);
-    const long long b = r / ks, p = b * PPB + j;
-    sig[i] = (j < PPB && p < np) ? sigma[(long long)(k0 + s) * np + p] : 0.f;
+    if (i >= nblk * M_KS * M_SROW) return;
+    const int s = (int)(i % M_KS);
+    const long long r = i / M_KS;
+    const int j = (int)(r % M_SROW);
+    const long long b = r / M_SROW, p = b * PPB + j;
+    sig[i] = (s < ks && j < PPB && p < np) ? sigma[(long long)(k0 + s) * np + p] : 0.f;
 }
 
 /* guarded fp64 recomputation of one target for one density vector (the rare zero-distance case, reading A4) */
@@ -143,12 +145,12 @@ __global__ void __launch_bounds__(M_THREADS, 1) panels_multi_kernel(const MultiP
     }
     __syncthreads();
 
-    const unsigned bytes_p = (unsigned)(SBH_P * sizeof(float4)), bytes_s = (unsigned)(KS * M_SROW * sizeof(float));
+    const unsigned bytes_p = (unsigned)(SBH_P * sizeof(float4)), bytes_s = (unsigned)(M_KS * M_SROW * sizeof(float));
     long long pu = 0, pblk = 0; /* producer (thread 0): next unit and its block */
     auto produce = [&](int stage) {
         mbar_expect_tx(&full[stage], bytes_p + bytes_s);
         tma_load_1d(&ring[stage][0], P.unit + pblk * SBH_P, bytes_p, &full[stage]);
-        tma_load_1d(&sring[stage][0], P.sig + pblk * (KS * M_SROW), bytes_s, &full[stage]);
+        tma_load_1d(&sring[stage][0], P.sig + pblk * (M_KS * M_SROW), bytes_s, &full[stage]);
         ++pu;
         if (++pblk == P.nblk) pblk = 0;
     };
@@ -242,9 +244,11 @@ __global__ void __launch_bounds__(M_THREADS, 1) panels_multi_kernel(const MultiP
                     }
                 }
                 /* 4 packed FMAs per density vector, panel and pair */
+                const float4 sg4 = *reinterpret_cast<const float4*>(ssig + pp * M_KS); /* one broadcast LDS.128 */
+                const float sgv[4] = {sg4.x, sg4.y, sg4.z, sg4.w};
 #pragma unroll
                 for (int s = 0; s < KS; ++s) {
-                    const float sg = ssig[s * M_SROW + pp];
+                    const float sg = sgv[s];
                     const u64 sg2 = pk(sg, sg);
 #pragma unroll
                     for (int p = 0; p < M_NP; ++p) {
@@ -376,7 +380,7 @@ extern "C" int obem_eval_panels_multi(obem_ctx* c, const float* d_sigma, int n_s
         const int ks = (n_sigma - k0 < M_KS) ? n_sigma - k0 : M_KS;
         P.k0 = k0;
         P.ks = ks;
-        const long long cells = nblk * ks * M_SROW;
+        const long long cells = nblk * M_KS * M_SROW;
         multi_sigma_kernel<<<(unsigned)ceil_div(cells, 256), 256, 0, st>>>(d_sigma, c->d_msig, np, nblk, k0, ks);
         OBEM_CUDA(c, cudaGetLastError());
         cudaError_t e = cudaSuccess;
