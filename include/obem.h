@@ -232,6 +232,18 @@ int obem_update_sigma_dynamic(obem_ctx* c, const int32_t* d_kind, const float* d
 int obem_eval_panels_multi(obem_ctx* c, const float* d_sigma, int n_sigma, const float* d_pts, int64_t m,
                            float* d_out, void* cuda_stream);
 
+/* The Shockley-Ramo signal sum, Eq (3.13) (section 3.4): the current induced on read-out electrode k
+ * by the moving particles,  i_k = sum_p q_p v_p . E_w^(k)(r_p),  "generated separately" for each particle type
+ * (PAPER.md:366):
+ *   d_xyzq [n][4] fp32 (only q is read);  d_vel [n][4] fp32 = vx, vy, vz [m/s] (4th lane ignored);
+ *   d_ew [n_electrodes][n][4] fp32 = the weighting field of electrode k at particle p [V/m for 1 V] -- the layout
+ *        obem_eval_panels_multi writes when its points are the particles;
+ *   d_out [n_electrodes][2] fp64 [A]: [k][0] = the particles with q < 0 (electrons), [k][1] = those with q > 0 (ions).
+ * Every term and every sum in fp64, fixed order: deterministic.  Sign as printed in Eq (3.13) (no minus sign).  A small
+ * library-owned buffer of partial sums grows (cudaMalloc) on the first call of a given size. */
+int obem_ramo_current(obem_ctx* c, const float* d_xyzq, const float* d_vel, const float* d_ew, int n_electrodes,
+                      int64_t n, double* d_out, void* cuda_stream);
+
 /* ----------------------------------------------------------------------------------------------------------
  * NEXT-2: numerical integrators, section 3.2.5 -- the consumers of the field evaluation.
  * State: d_xyzq [n][4] fp32 = x, y, z [m], q [C];  d_vel [n][4] fp32 = vx, vy, vz [m/s], m [kg] (m = 0: immobile).

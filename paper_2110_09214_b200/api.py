@@ -57,6 +57,7 @@ SIGNATURES = {
                                                  ctypes.c_void_p]),
     "obem_get_panel_normals": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_void_p]),
     "obem_eval_panels_multi": (ctypes.c_int, [ctypes.c_void_p, _c_fp, ctypes.c_int, _c_fp, _i64, _c_fp, ctypes.c_void_p]),
+    "obem_ramo_current": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, ctypes.c_int, _i64, _c_fp, ctypes.c_void_p]),
     # NEXT-2: recombination by-product of the N-body pass
     "obem_eval_at_charges_partners": (ctypes.c_int, [ctypes.c_void_p, _c_fp, _c_fp, _c_fp, ctypes.c_uint,
                                                      ctypes.c_void_p]),
@@ -423,6 +424,21 @@ class Context:
                                                 pts.data_ptr() if m else None, m,
                                                 out.data_ptr() if (k and m) else None, _stream_ptr(stream)),
                     "obem_eval_panels_multi")
+        return out
+
+    def ramo_current(self, xyzq, vel, ew, stream=None):
+        """Eq (3.13): xyzq [N,4], vel [N,4], ew [K,N,4] float32 -> [K,2] float64 (electrons, ions) [A]."""
+        torch = _torch()
+        n, k = int(xyzq.shape[0]), int(ew.shape[0])
+        if n and k:
+            _dev_f32(xyzq, "xyzq", (4,)), _dev_f32(vel, "vel", (4,)), _dev_f32(ew, "ew", (4,))
+            if vel.shape[0] != n or tuple(ew.shape) != (k, n, 4):
+                raise ValueError("vel must be [N, 4] and ew [K, N, 4]")
+        out = torch.empty((k, 2), dtype=torch.float64, device="cuda:%d" % self.device)
+        ok = n > 0 and k > 0
+        self._check(_lib.obem_ramo_current(self._h, xyzq.data_ptr() if ok else None, vel.data_ptr() if ok else None,
+                                           ew.data_ptr() if ok else None, k, n, out.data_ptr() if k else None,
+                                           _stream_ptr(stream)), "obem_ramo_current")
         return out
 
     def get_panel_normals(self, stream=None):

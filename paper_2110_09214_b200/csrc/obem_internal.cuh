@@ -267,6 +267,8 @@ struct obem_ctx {
     float* d_msig = nullptr;     /* one pass's density vectors, blocked */
     size_t munit_cap = 0, msig_cap = 0;
     long long munit_geom = -1;   /* geom_version d_munit was built for */
+    double* d_ramo = nullptr;    /* [K][blocks][2] partial sums of obem_ramo_current */
+    size_t ramo_cap = 0;
     /* obem_map.cu */
     float4* d_map_pts = nullptr; /* node coordinates of the last obem_field_map */
     size_t map_pts_cap = 0;      /* bytes */

@@ -296,6 +296,50 @@ __global__ void __launch_bounds__(M_THREADS, 1) panels_multi_kernel(const MultiP
     }
 }
 
+/*
+ * The Shockley-Ramo signal sum, Eq (3.13): i_k = sum_p q_p v_p . E_w^(k)(r_p), separately for the
+ * particles with q < 0 and with q > 0 ("the signals created by each type are generated separately").
+ * ew [K][n] is what obem_eval_panels_multi writes for K weighting-field density vectors at the charges.  fp32 inputs,
+ * every term and every sum in fp64, fixed summation order (strided per thread, tree per block, blocks in order): the
+ * result is deterministic.  Bound: HBM (16 B of E_w per particle and electrode; q and v come from L2 after the first
+ * electrode).  Grid: (blocks, K).
+ */
+constexpr int R_THREADS = 256;
+__global__ void __launch_bounds__(R_THREADS) ramo_partial_kernel(const float4* __restrict__ xyzq, const float4* __restrict__ vel,
+                                                                 const float4* __restrict__ ew, long long n, long long chunk,
+                                                                 double* __restrict__ part)
+{
+    __shared__ double red[2][R_THREADS];
+    const int tid = threadIdx.x, k = blockIdx.y;
+    const long long i0 = (long long)blockIdx.x * chunk, i1 = (i0 + chunk < n) ? i0 + chunk : n;
+    double neg = 0.0, pos = 0.0;
+    for (long long i = i0 + tid; i < i1; i += R_THREADS) {
+        const float q = xyzq[i].w;
+        const float4 v = vel[i], e = ew[(long long)k * n + i];
+        const double term = (double)q * ((double)v.x * (double)e.x + (double)v.y * (double)e.y + (double)v.z * (double)e.z);
+        if (q < 0.f) neg += term;
+        else if (q > 0.f) pos += term;
+    }
+    red[0][tid] = neg, red[1][tid] = pos;
+    __syncthreads();
+    for (int h = R_THREADS / 2; h > 0; h >>= 1) {
+        if (tid < h) red[0][tid] += red[0][tid + h], red[1][tid] += red[1][tid + h];
+        __syncthreads();
+    }
+    if (tid == 0) {
+        part[((size_t)k * gridDim.x + blockIdx.x) * 2 + 0] = red[0][0];
+        part[((size_t)k * gridDim.x + blockIdx.x) * 2 + 1] = red[1][0];
+    }
+}
+__global__ void ramo_final_kernel(const double* __restrict__ part, int blocks, int K, double* __restrict__ out)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= K) return;
+    double neg = 0.0, pos = 0.0;
+    for (int b = 0; b < blocks; ++b) neg += part[((size_t)k * blocks + b) * 2], pos += part[((size_t)k * blocks + b) * 2 + 1];
+    out[2 * k] = neg, out[2 * k + 1] = pos;
+}
+
 template <int KS>
 cudaError_t launch_pass(obem_ctx* c, const MultiParams& P, cudaStream_t st)
 {
@@ -319,6 +363,9 @@ void obem_multi_free(obem_ctx* c)
 {
     if (c->d_munit) cudaFree(c->d_munit);
     if (c->d_msig) cudaFree(c->d_msig);
+    if (c->d_ramo) cudaFree(c->d_ramo);
+    c->d_ramo = nullptr;
+    c->ramo_cap = 0;
     c->d_munit = nullptr;
     c->d_msig = nullptr;
     c->munit_cap = c->msig_cap = 0;
@@ -393,5 +440,39 @@ extern "C" int obem_eval_panels_multi(obem_ctx* c, const float* d_sigma, int n_s
         OBEM_CUDA(c, e);
         c->launches += 2;
     }
+    return OBEM_OK;
+}
+
+extern "C" int obem_ramo_current(obem_ctx* c, const float* d_xyzq, const float* d_vel, const float* d_ew, int n_electrodes,
+                                 int64_t n, double* d_out, void* cuda_stream)
+{
+    if (!c || n_electrodes < 0 || n < 0) return OBEM_EINVAL;
+    if (n_electrodes == 0) return OBEM_OK;
+    if (!d_out || (((uintptr_t)d_out) & 7u)) return OBEM_EINVAL;
+    if (n > 0 && (!d_xyzq || !d_vel || !d_ew || !aligned16(d_xyzq) || !aligned16(d_vel) || !aligned16(d_ew))) return OBEM_EINVAL;
+    DeviceGuard g(c->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (n == 0) {
+        OBEM_CUDA(c, cudaMemsetAsync(d_out, 0, (size_t)n_electrodes * 2 * sizeof(double), st));
+        return OBEM_OK;
+    }
+    long long blocks = ceil_div(n, 4LL * R_THREADS);
+    if (blocks > 1024) blocks = 1024;
+    const long long chunk = ceil_div(ceil_div(n, blocks), R_THREADS) * R_THREADS;
+    blocks = ceil_div(n, chunk);
+    const size_t need = (size_t)n_electrodes * (size_t)blocks * 2;
+    if (need > c->ramo_cap) {
+        double* p = nullptr;
+        OBEM_CUDA(c, cudaMalloc(&p, need * sizeof(double)));
+        if (c->d_ramo) cudaFree(c->d_ramo);
+        c->d_ramo = p;
+        c->ramo_cap = need;
+    }
+    ramo_partial_kernel<<<dim3((unsigned)blocks, (unsigned)n_electrodes), R_THREADS, 0, st>>>(
+        (const float4*)d_xyzq, (const float4*)d_vel, (const float4*)d_ew, n, chunk, c->d_ramo);
+    OBEM_CUDA(c, cudaGetLastError());
+    ramo_final_kernel<<<(unsigned)ceil_div(n_electrodes, 64), 64, 0, st>>>(c->d_ramo, (int)blocks, n_electrodes, d_out);
+    OBEM_CUDA(c, cudaGetLastError());
+    c->launches += 2;
     return OBEM_OK;
 }

@@ -131,3 +131,70 @@ def test_multi_sigma_config3_full_size_sampled(torch_cuda, api, ctx, ref):
     for s in range(4):
         _, op = ref.eval_field(verts=wl.verts, sigma=sig[s], targets=wl.xyzq[idx], flags=ref.PANELS)
         assert_parity(out[s][idx], op, "cfg3 multi-sigma vector %d" % s)
+
+
+# --------------------------------------------------------------------------------------------------
+# Shockley-Ramo signal sum, Eq (3.13)
+# --------------------------------------------------------------------------------------------------
+QE = 1.602176634e-19
+EPS0 = 8.8541878128e-12
+
+
+def test_ramo_current_matches_the_oracle(torch_cuda, api, ctx):
+    from oracle import ramo
+    torch = torch_cuda
+    rng = np.random.default_rng([53, 1])
+    for n, k in ((50021, 3), (1, 1), (300, 5)):
+        xyzq = np.zeros((n, 4), dtype=np.float32)
+        xyzq[:, 3] = rng.choice([-QE, QE, 2 * QE, 0.0], n, p=[0.5, 0.3, 0.1, 0.1])
+        vel = np.zeros((n, 4), dtype=np.float32)
+        vel[:, :3] = rng.normal(0, 1e5, (n, 3))
+        vel[:, 3] = 9.1e-31                                         # the mass lane is ignored
+        ew = rng.normal(0, 1e3, (k, n, 4)).astype(np.float32)
+        a = ctx.ramo_current(dev(torch, xyzq), dev(torch, vel), dev(torch, ew))
+        b = ctx.ramo_current(dev(torch, xyzq), dev(torch, vel), dev(torch, ew))
+        assert torch.equal(a, b)                                    # fixed summation order
+        exp = ramo.ramo_current(xyzq[:, 3], vel[:, :3], ew[:, :, :3])
+        scale = np.einsum("p,kp->k", np.abs(xyzq[:, 3].astype(np.float64)),
+                          np.abs(vel[None, :, :3].astype(np.float64) * ew[:, :, :3].astype(np.float64)).sum(axis=2))
+        assert np.all(np.abs(a.cpu().numpy() - exp) <= 1e-12 * scale[:, None] + 1e-300), (n, k)
+    assert tuple(ctx.ramo_current(dev(torch, xyzq[:0]), dev(torch, vel[:0]), dev(torch, ew[:, :0])).shape) == (5, 2)
+    assert torch.all(ctx.ramo_current(dev(torch, xyzq[:0]), dev(torch, vel[:0]), dev(torch, ew[:, :0])) == 0)
+
+
+def test_weighting_field_to_signal_chain_on_parallel_plates(torch_cuda, api, ctx, ref):
+    """The whole read-out chain on the geometry of the paper's Figure 9 (a parallel-plate counter): two plates, the
+    read-out one at 1 V -- surface densities +-eps0/d away from the rims -- evaluated with obem_eval_panels_multi at
+    the particles, then Eq (3.13).  Against the oracle chain (fp64 panel sums, then the Ramo oracle) at the path's
+    tolerance, and against the closed form i = N e v_z |E_w| with the on-axis field of the finite plates."""
+    from oracle import ramo
+    torch = torch_cuda
+    d, half = 5.0 * UM, 50.0 * UM
+    bottom = W.plane_mesh(-half, half, -half, half, 0.0, 32, 32)
+    top = W.plane_mesh(-half, half, -half, half, d, 32, 32)
+    verts = np.concatenate([bottom, top]).astype(np.float32)
+    npl = bottom.shape[0]
+    sig_w = np.concatenate([np.full(npl, -EPS0 / d), np.full(npl, +EPS0 / d)]).astype(np.float32)   # read-out = top
+    sig_other = (-sig_w).astype(np.float32)                                                            # read-out = bottom
+    rng = np.random.default_rng([53, 2])
+    n = 4000
+    xyzq = np.zeros((n, 4), dtype=np.float32)
+    xyzq[:, :2] = rng.uniform(-10 * UM, 10 * UM, (n, 2))                 # the central fifth of the plates
+    xyzq[:, 2] = rng.uniform(1.0 * UM, 4.0 * UM, n)
+    xyzq[:, 3] = -QE
+    vel = np.zeros((n, 4), dtype=np.float32)
+    vel[:, 2] = 1.0e5
+    vel[:, :2] = rng.normal(0, 3e4, (n, 2))
+    ctx.set_panels(dev(torch, verts), dev(torch, sig_w))
+    sig = np.stack([sig_w, sig_other])
+    ew = ctx.eval_panels_multi(dev(torch, sig), dev(torch, xyzq))
+    i_gpu = ctx.ramo_current(dev(torch, xyzq), dev(torch, vel), ew).cpu().numpy()
+    ew_ref = np.stack([ref.eval_field(verts=verts, sigma=s, targets=xyzq, flags=ref.PANELS)[1] for s in sig])
+    i_ref = ramo.ramo_current(xyzq[:, 3], vel[:, :3], ew_ref[:, :, :3])
+    assert np.allclose(i_gpu[:, 0], i_ref[:, 0], rtol=2e-5, atol=0)
+    assert np.all(i_gpu[:, 1] == 0)                                       # no ions
+    # closed form: electrons towards the 1 V plate induce + N e v_z |E_w|; between two SQUARE plates of half-width a the
+    # field on the axis is (sigma/eps0) (1 - sqrt(2) d / (pi a)) to first order in d/a (the on-axis formula of a
+    # uniformly charged rectangle, pin P7, for both plates): 0.955/d here, within +-0.5 % over the central fifth
+    closed = n * QE * 1.0e5 / d * (1.0 - np.sqrt(2.0) * d / (np.pi * half))
+    assert abs(i_gpu[0, 0] / closed - 1.0) < 0.01 and abs(i_gpu[1, 0] / closed + 1.0) < 0.01
