@@ -702,7 +702,16 @@ def bench_next1(torch, api, ctx, wl, timed, dev, t_panels):
                              "Ginteractions_per_s_per_vector_equivalent": 4 * inter / t_m4 / 1e9,
                              "frac_fp32_peak_of_executed_work": FLOP_PER_INTERACTION * inter * (103.0 / 87.0) / t_m4 / 1e12
                              / peak_flops, "bound": "alu"}
-    del sig4, out4, pts
+    # Eq (3.13) on that pass's output: the induced currents of the 4 electrodes (HBM-bound, launch-latency scale)
+    vel = torch.zeros((n, 4), dtype=torch.float32, device=dev)
+    vel[:, 2] = 1.0e5
+    t_ramo = timed(lambda: ctx.ramo_current(pts, vel, out4), reps=5)
+    peak_hbm, src_hbm = hbm_peak_gbs()
+    ramo_bytes = n * (16 * 4 + 32)
+    res["ramo_current_4"] = {"s": t_ramo, "bound": "hbm (two launches: latency-bound at this size)",
+                             "algorithmic_bytes": ramo_bytes, "achieved": ramo_bytes / t_ramo / 1e9, "peak": peak_hbm,
+                             "unit": "GB/s", "frac": ramo_bytes / t_ramo / 1e9 / peak_hbm, "peak_source": src_hbm}
+    del sig4, out4, pts, vel
     free, _ = torch.cuda.mem_get_info()
     ng = npan
     while ng > 1024 and 4 * ng * ng > 0.6 * free:

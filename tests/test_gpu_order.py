@@ -263,3 +263,25 @@ def test_e_only_is_bit_identical_in_E_and_zero_in_phi(torch_cuda, api, ctx, ref)
     with pytest.raises(api.ObemError) as e:
         ctx.eval_at_charges_partners(flags=api.NBODY | api.NO_PHI)
     assert e.value.status == -1
+
+
+def test_pair_order_config4_full_size_sampled(torch_cuda, api, ctx, ref):
+    """BASELINE.json configs[3] (4,194,304 charges in two clouds 2 mm apart, 262,144 panels) in pair-creation order:
+    the largest charge set, where the class order puts 2.1 M electrons before 2.1 M ions and the species sums reach
+    ~200 x the net potential (the case that needs the fp64 second accumulation level)."""
+    torch = torch_cuda
+    wl = W.pair_creation_order(W.make_workload(4))
+    ctx.set_softening(wl.eps_pp, wl.eps_panel)
+    ctx.set_panels(dev(torch, wl.verts), dev(torch, wl.sigma))
+    ctx.set_charges(dev(torch, wl.xyzq))
+    g = ctx.eval_at_charges(flags=api.NBODY | api.PANELS)
+    torch.cuda.synchronize()
+    g = g.cpu().numpy()
+    assert np.isfinite(g).all()
+    rng = np.random.default_rng([23, 4])
+    mag = np.linalg.norm(g[:, :3], axis=1)
+    idx = np.unique(np.concatenate([rng.choice(wl.n_charges, 384, replace=False), np.argsort(mag)[-32:],
+                                    np.argsort(np.abs(g[:, 3]))[:32], [0, wl.n_charges - 1]]))
+    on, op = ref.eval_field(xyzq=wl.xyzq, verts=wl.verts, sigma=wl.sigma, targets=wl.xyzq[idx],
+                            self_index=idx.astype(np.int64), eps_pp=wl.eps_pp, eps_panel=wl.eps_panel)
+    assert_parity(g[idx], on + op, "cfg4 pair order, sampled")
