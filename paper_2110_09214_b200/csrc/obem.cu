@@ -928,7 +928,7 @@ __device__ __forceinline__ long long cta_of(long long u, long long U, long long 
 /* Tiles that were split between CTAs: sum their partials (fixed order, fp64), scale, write.  One CTA per (tile,
  * target slot k): thread t owns target tile * tt + k * THREADS + t.  The unit ranges of the CTAs that share the tile
  * are formed once per CTA (one 64-bit division per thread, none in the summation loop). */
-__global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P, const int G)
+__global__ void __launch_bounds__(THREADS, 3) obem_fixup_kernel(const EvalParams P, const int G)
 {
     extern __shared__ long long cta_u0[]; /* [cB - cA + 2] first unit of CTAs cA .. cB + 1 */
     const long long tile = blockIdx.x;
@@ -951,24 +951,42 @@ __global__ void __launch_bounds__(THREADS) obem_fixup_kernel(const EvalParams P,
     double ex = 0.0, ey = 0.0, ez = 0.0, ph = 0.0;
     float tm = __int_as_float(0x7f800000);
     int tb = -1;
-    for (long long c = cA; c <= cB; ++c) {
-        const long long c0 = cta_u0[c - cA], c1 = cta_u0[c - cA + 1];
-        if (c0 >= c1) continue;
-        const int slot = (c0 >= uA && c0 <= uB) ? 0 : 1; /* the CTA's range STARTS inside this tile */
-        if (P.trk_out) { /* CTAs in ascending block order: strict < keeps the lowest block on ties */
-            const float2 t = P.trk_ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
-            if (t.x < tm) {
-                tm = t.x;
-                tb = __float_as_int(t.y);
+    /* FIX_B partials in flight per thread (their loads are independent; the sums below keep the order of c) */
+    constexpr int FIX_B = 4;
+    for (long long cb = cA; cb <= cB; cb += FIX_B) {
+        double2 v0[FIX_B], v1[FIX_B];
+        float2 t[FIX_B];
+        bool ok[FIX_B];
+#pragma unroll
+        for (int j = 0; j < FIX_B; ++j) {
+            const long long c = cb + j;
+            ok[j] = false;
+            if (c <= cB) {
+                const long long c0 = cta_u0[c - cA], c1 = cta_u0[c - cA + 1];
+                ok[j] = c0 < c1;
+                const int slot = (c0 >= uA && c0 <= uB) ? 0 : 1; /* the CTA's range STARTS inside this tile */
+                if (ok[j]) {
+                    if (P.trk_out) t[j] = P.trk_ws[((size_t)c * 2 + slot) * P.ws_stride + (size_t)k * THREADS + tid];
+                    const double2* v = reinterpret_cast<const double2*>(
+                        P.ws + (((size_t)c * 2 + slot) * TT_MAX + (size_t)k * THREADS + tid) * 4);
+                    v0[j] = v[0];
+                    v1[j] = v[1];
+                }
             }
         }
-        const double2* v =
-            reinterpret_cast<const double2*>(P.ws + (((size_t)c * 2 + slot) * TT_MAX + (size_t)k * THREADS + tid) * 4);
-        const double2 v0 = v[0], v1 = v[1];
-        ex += v0.x;
-        ey += v0.y;
-        ez += v1.x;
-        ph += v1.y;
+#pragma unroll
+        for (int j = 0; j < FIX_B; ++j) {
+            if (!ok[j]) continue;
+            /* CTAs in ascending block order: strict < keeps the lowest block on ties */
+            if (P.trk_out && t[j].x < tm) {
+                tm = t[j].x;
+                tb = __float_as_int(t[j].y);
+            }
+            ex += v0[j].x;
+            ey += v0[j].y;
+            ez += v1[j].x;
+            ph += v1[j].y;
+        }
     }
     const long long oi = P.out_idx ? (long long)P.out_idx[i] : i;
     float4 o = make_float4((float)(KE_D * ex), (float)(KE_D * ey), (float)(KE_D * ez), (float)(KE_D * ph));
