@@ -1,0 +1,176 @@
+"""Seeded random cases of libobem.so against the fp64 oracle: sizes on and around the block (256), tile (512 / 2048)
+and grid boundaries, every flag combination, every storage order of the charges (species order, interleaved, several
+ion charges, one sign, arbitrary macro-particle weights with zeros), unsoftened coincident pairs, target ranges, free
+points (some on charges), recombination partners, the NN path at theta = 0.  `pytest -m gpu`.
+
+E is held to the bars of tests/parity_metrics.py in every case.  phi too, with one addition: panels with surface
+charges of RANDOM sign (no electrode looks like that, but nothing forbids it) make phi at a target a sum that cancels
+to 1/200 of the sum of its terms' magnitudes and less, and then "relative to max(|phi|, 1e-2 rms)" asks for more than
+fp32 terms can give.  The forward error of a sum of fp32-rounded terms is bounded by gamma * sum_j |term_j| (each term:
+the reciprocal square root within 2 ulp and four roundings, gamma = 3e-7); the oracle gives sum_j |term_j| exactly
+(the same evaluation with |q| and |sigma|), so a phi that misses the relative bar must meet that absolute one.
+Measured on 2,791 such cases (24,516 comparisons): |dphi| ~ 2e-8 * sum|terms| rms, no E failure.
+"""
+import numpy as np
+import pytest
+
+from parity_metrics import PHI_FLOOR, TOL_MAX_REL, TOL_REL_L2, field_errors
+
+pytestmark = pytest.mark.gpu
+
+UM = 1e-6
+QE = 1.602176634e-19
+GAMMA = 3e-7
+
+N_EDGES = [1, 2, 3, 31, 255, 256, 257, 511, 512, 513, 1023, 1024, 1025, 2047, 2048, 2049, 4095, 4096, 4097, 8191, 8193]
+P_EDGES = [0, 0, 1, 2, 33, 34, 35, 67, 68, 69, 511, 512, 1000]
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("the gpu-marked tests need a CUDA device (there is no CPU fallback)")
+    return torch
+
+
+@pytest.fixture(scope="module")
+def api(torch_cuda):
+    from paper_2110_09214_b200 import api as _api
+    return _api
+
+
+def make_case(rng):
+    n = int(rng.choice(N_EDGES)) if rng.random() < 0.6 else int(rng.integers(1, 9000))
+    npan = int(rng.choice(P_EDGES)) if rng.random() < 0.7 else int(rng.integers(1, 1200))
+    xyzq = np.zeros((n, 4), dtype=np.float32)
+    shape = int(rng.integers(0, 3))
+    if shape == 0:
+        xyzq[:, :3] = rng.uniform(0, 80 * UM, (n, 3))
+    elif shape == 1:
+        xyzq[:, :3] = rng.normal(0, 1, (n, 3)) * np.array([30 * UM, 30 * UM, 5 * UM]) + 40 * UM
+    else:
+        xyzq[:, :3] = rng.normal(0, 1, (n, 3)) * 10 * UM + 40 * UM
+    order = int(rng.integers(0, 5))
+    if order == 0:          # species order: all electrons, then all ions
+        k = int(rng.integers(0, n + 1))
+        xyzq[:k, 3] = -QE
+        xyzq[k:, 3] = QE
+    elif order == 1:        # pair-creation order: signs interleaved
+        xyzq[:, 3] = rng.choice([-QE, QE], n)
+    elif order == 2:        # several ion charges
+        xyzq[:, 3] = rng.choice([-QE, QE, 2 * QE, 3 * QE], n)
+    elif order == 3:        # one sign only
+        xyzq[:, 3] = QE if rng.random() < 0.5 else -QE
+    else:                   # macro-particles of arbitrary weight, some of weight zero
+        xyzq[:, 3] = rng.normal(0, 1, n) * QE * 100
+        xyzq[rng.random(n) < 0.05, 3] = 0.0
+    if shape == 2 and order in (0, 1):
+        xyzq[xyzq[:, 3] > 0, 2] += 60 * UM      # the ions' tail apart from the electrons' head
+    verts = (rng.uniform(0, 80 * UM, (npan, 1, 3)) + rng.uniform(-2 * UM, 2 * UM, (npan, 3, 3))).astype(np.float32)
+    if npan:
+        verts[..., 2] += 125 * UM
+    sigma = rng.normal(0, 1e-5, npan).astype(np.float32)
+    if rng.random() < 0.5:
+        sigma = np.abs(sigma)                    # an electrode: one sign
+    eps_pp = float(rng.choice([0.0, 0.05 * UM, 0.5 * UM]))
+    eps_pan = float(rng.choice([0.0, 0.0, 0.1 * UM]))
+    if eps_pp == 0.0 and n > 40 and rng.random() < 0.5:
+        for _ in range(int(rng.integers(1, 4))):     # different charges at one position (reading A4)
+            a, b = rng.integers(0, n, 2)
+            xyzq[a, :3] = xyzq[b, :3]
+    return xyzq, verts, sigma, eps_pp, eps_pan
+
+
+def check(got, want, want_abs, what, e_only=False):
+    """want_abs[:, 3] = sum of the magnitudes of the terms of want[:, 3] (the oracle on |q|, |sigma|)."""
+    got = np.asarray(got, dtype=np.float64)
+    assert got.shape == want.shape, what
+    assert np.isfinite(got).all(), "%s: non-finite GPU output" % what
+    if got.shape[0] == 0:
+        return
+    if e_only:                                   # OBEM_NO_PHI: column 3 is not part of the result
+        got = got.copy()
+        got[:, 3] = want[:, 3]
+    e = field_errors(got, want)
+    assert e["E_rel_l2"] <= TOL_REL_L2, "%s: E rel-L2 %.3e" % (what, e["E_rel_l2"])
+    assert e["E_max_rel"] <= TOL_MAX_REL, "%s: E per-target %.3e" % (what, e["E_max_rel"])
+    dphi = np.abs(got[:, 3] - want[:, 3])
+    pabs = want_abs[:, 3]
+    rms = float(np.sqrt((want[:, 3] ** 2).mean()))
+    bar = np.maximum(TOL_MAX_REL * np.maximum(np.abs(want[:, 3]), PHI_FLOOR * rms), GAMMA * pabs)
+    worst = int(np.argmax(dphi - bar))
+    assert (dphi <= bar).all(), "%s: phi target %d: |dphi| %.3e, |phi| %.3e, rms %.3e, sum|terms| %.3e" % (
+        what, worst, dphi[worst], abs(want[worst, 3]), rms, pabs[worst])
+    l2_bar = max(TOL_REL_L2 * float(np.sqrt((want[:, 3] ** 2).sum())), GAMMA * float(np.sqrt((pabs ** 2).sum())))
+    assert float(np.sqrt((dphi ** 2).sum())) <= l2_bar, "%s: phi L2 %.3e > %.3e" % (
+        what, float(np.sqrt((dphi ** 2).sum())), l2_bar)
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_cases_against_the_oracle(torch_cuda, api, ref, seed):
+    torch = torch_cuda
+    rng = np.random.default_rng([2110, 9214, seed])
+
+    def dev(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    for case in range(10):
+        xyzq, verts, sigma, eps_pp, eps_pan = make_case(rng)
+        n, npan = xyzq.shape[0], verts.shape[0]
+        what = "seed %d case %d (n %d, panels %d, eps %g / %g, %d kinds of charge)" % (
+            seed, case, n, npan, eps_pp, eps_pan, len(np.unique(xyzq[:, 3])))
+        xabs = xyzq.copy()
+        xabs[:, 3] = np.abs(xabs[:, 3])
+        on, op = ref.eval_field(xyzq=xyzq, verts=verts, sigma=sigma, eps_pp=eps_pp, eps_panel=eps_pan)
+        an, ap = ref.eval_field(xyzq=xabs, verts=verts, sigma=np.abs(sigma), eps_pp=eps_pp, eps_panel=eps_pan)
+        with api.Context(0) as ctx:
+            ctx.set_softening(eps_pp, eps_pan)
+            if npan:
+                ctx.set_panels(dev(verts), dev(sigma))
+            ctx.set_charges(dev(xyzq))
+            combos = [(api.NBODY, on, an)]
+            if npan:
+                combos += [(api.PANELS, op, ap), (api.NBODY | api.PANELS, on + op, an + ap)]
+            for fl, want, wabs in combos:
+                g = ctx.eval_at_charges(flags=fl).cpu().numpy()
+                check(g, want, wabs, what + " at the charges, flags %d" % fl)
+                g = ctx.eval_at_charges(flags=fl | api.NO_PHI).cpu().numpy()
+                check(g, want, wabs, what + " at the charges, E only, flags %d" % fl, e_only=True)
+            fl, want, wabs = combos[-1]
+            first = int(rng.integers(0, n))
+            count = int(rng.integers(0, n - first + 1))
+            g = ctx.eval_at_charges_range(first, count, flags=fl).cpu().numpy()
+            check(g, want[first:first + count], wabs[first:first + count], what + " range [%d, +%d)" % (first, count))
+            m = int(rng.choice([1, 7, 255, 256, 257, 2048, 2049]))
+            pts = np.zeros((m, 4), dtype=np.float32)
+            pts[:, :3] = rng.uniform(-10 * UM, 90 * UM, (m, 3))
+            k = min(m, n, 5)
+            pts[:k, :3] = xyzq[rng.integers(0, n, k), :3]
+            qn, qp = ref.eval_field(xyzq=xyzq, verts=verts, sigma=sigma, targets=pts, self_index=None,
+                                    eps_pp=eps_pp, eps_panel=eps_pan)
+            bn, bp = ref.eval_field(xyzq=xabs, verts=verts, sigma=np.abs(sigma), targets=pts, self_index=None,
+                                    eps_pp=eps_pp, eps_panel=eps_pan)
+            g = ctx.eval_at_points(dev(pts), flags=fl).cpu().numpy()
+            check(g, qn + qp, bn + bp, what + " at %d points" % m)
+            if n >= 2 and not np.any(xyzq[:, 3] == 0):
+                out, pd, pj = ctx.eval_at_charges_partners(flags=api.NBODY)
+                check(out.cpu().numpy(), on, an, what + " partners' field")
+                d, j = ref.nearest_opposite(xyzq)
+                pd = pd.cpu().numpy().astype(np.float64)
+                pj = pj.cpu().numpy().astype(np.int64)
+                none = np.isinf(d)
+                assert np.array_equal(np.isinf(pd), none) and np.all(pj[none] == -1), what
+                # distance: fp64 on the fp32 coordinates, returned as fp32
+                assert np.all(np.abs(pd[~none] - d[~none]) <= 1e-6 * d[~none]), what
+                # index: the oracle's, except between candidates at the same distance to within that rounding
+                other = (pj != j) & ~none
+                if other.any():
+                    dd = np.linalg.norm(xyzq[other, :3].astype(np.float64) - xyzq[pj[other], :3].astype(np.float64),
+                                        axis=1)
+                    assert np.all(np.abs(dd - d[other]) <= 1e-6 * d[other]), what
+                    assert np.all(np.sign(xyzq[pj[other], 3]) == -np.sign(xyzq[other, 3])), what
+            if case % 2 == 0:
+                ctx.set_nn_theta(0.0)            # the NN lists with nothing far: the exact sum through the LIST kernel
+                g = ctx.eval_at_charges_nn(flags=api.NBODY).cpu().numpy()
+                check(g, on, an, what + " NN path at theta 0")
