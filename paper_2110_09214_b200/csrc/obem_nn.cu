@@ -21,6 +21,7 @@
  * Every step is enqueued on the caller's stream; nothing is read back to the host (all sizes follow from n).
  * Part of libobem.so; shares nothing with oracle/.
  */
+#include <cub/block/block_radix_sort.cuh>
 #include <cub/device/device_radix_sort.cuh>
 
 #include "obem_internal.cuh"
@@ -174,6 +175,123 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
     keys[i] = ((u64k)rank << 32) | (u64k)low; /* `level` bits of segment rank + 32 of coordinate: 4-6 radix passes */
 }
 
+/*
+ * The last levels of the k-d order, one CTA per segment.  Once every segment holds at most KD_LOCAL_LEAVES leaves
+ * (4096 charges) the remaining cuts touch nothing outside it: the CTA keeps the segment's 4096 (key, index) pairs in
+ * registers and runs the same rounds as the global loop -- boxes of the current sub-segments, axis = first of the
+ * largest extents (fp64), STABLE sort by (sub-segment rank, ordered coordinate), cut at nn_split -- with a block-wide
+ * radix sort instead of a device-wide one: the same order, bit for bit (a stable sort by the same keys), in one launch
+ * instead of three launches + 5-6 radix passes per level.  CTA k takes the segment whose l0-bit path is k.
+ */
+constexpr int KD_LOCAL_LEAVES = 16, KD_THREADS = 256, KD_ITEMS = KD_LOCAL_LEAVES * LEAF / KD_THREADS;
+constexpr int KD_MAX_SUB = KD_LOCAL_LEAVES / 2; /* sub-segments that can still be cut in the last round */
+typedef cub::BlockRadixSort<u64k, KD_THREADS, KD_ITEMS, int, 6> KdSort; /* 6-bit digits: 6 passes over 33-36 key bits */
+
+__global__ void __launch_bounds__(KD_THREADS, 2) nn_kd_local_kernel(const float4* __restrict__ x, int* __restrict__ perm,
+                                                                 long long n, int l0, int levels)
+{
+    __shared__ typename KdSort::TempStorage sort_tmp;
+    __shared__ unsigned smin[2 * KD_MAX_SUB][3], smax[2 * KD_MAX_SUB][3];
+    long long a = 0, b = n;
+    for (int t = 0; t < l0; ++t) {
+        const unsigned bit = ((unsigned)blockIdx.x >> (l0 - 1 - t)) & 1u;
+        if (b - a <= LEAF) {
+            if (bit) return; /* a final segment has path bits 0 from there on */
+            continue;
+        }
+        const long long m = nn_split(a, b);
+        if (bit) a = m;
+        else b = m;
+    }
+    if (b - a <= LEAF) return; /* final already: its order stays */
+    const int m = (int)(b - a), tid = threadIdx.x;
+    u64k key[KD_ITEMS];
+    int val[KD_ITEMS];
+#pragma unroll
+    for (int j = 0; j < KD_ITEMS; ++j) {
+        const int p = tid * KD_ITEMS + j;
+        val[j] = p < m ? perm[a + p] : -1;
+    }
+    /* sub-segment of position p (relative to a) after t more cuts: [ua, ub), its t-bit path r */
+    auto sub_of = [&](const int p, const int t, int& ua, int& ub, unsigned& r) {
+        ua = 0, ub = m, r = 0u;
+        for (int q = 0; q < t; ++q) {
+            r <<= 1;
+            if (ub - ua <= LEAF) continue;
+            const int mid = ua + LEAF * (((ub - ua + LEAF - 1) / LEAF + 1) / 2); /* nn_split: a is a multiple of LEAF */
+            if (p < mid) ub = mid;
+            else ua = mid, r |= 1u;
+        }
+    };
+    for (int t = 0; t < levels - l0; ++t) {
+        if (tid < 2 * KD_MAX_SUB * 3) {
+            (&smin[0][0])[tid] = 0xffffffffu;
+            (&smax[0][0])[tid] = 0u;
+        }
+        __syncthreads();
+        /* boxes: a thread's 16 consecutive positions lie in at most two sub-segments */
+        unsigned run_rank = 0xffffffffu, bmin[3], bmax[3];
+#pragma unroll
+        for (int j = 0; j < KD_ITEMS; ++j) {
+            const int p = tid * KD_ITEMS + j;
+            if (p >= m) continue;
+            int ua, ub;
+            unsigned r;
+            sub_of(p, t, ua, ub, r);
+            if (ub - ua <= LEAF) continue; /* final */
+            const float4 v = x[val[j]];
+            const unsigned k0 = nn_ordered(v.x), k1 = nn_ordered(v.y), k2 = nn_ordered(v.z);
+            if (r != run_rank) {
+                if (run_rank != 0xffffffffu) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) atomicMin(&smin[run_rank][d], bmin[d]), atomicMax(&smax[run_rank][d], bmax[d]);
+                }
+                run_rank = r;
+                bmin[0] = bmax[0] = k0, bmin[1] = bmax[1] = k1, bmin[2] = bmax[2] = k2;
+            } else {
+                bmin[0] = min(bmin[0], k0), bmax[0] = max(bmax[0], k0);
+                bmin[1] = min(bmin[1], k1), bmax[1] = max(bmax[1], k1);
+                bmin[2] = min(bmin[2], k2), bmax[2] = max(bmax[2], k2);
+            }
+        }
+        if (run_rank != 0xffffffffu) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) atomicMin(&smin[run_rank][d], bmin[d]), atomicMax(&smax[run_rank][d], bmax[d]);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int j = 0; j < KD_ITEMS; ++j) {
+            const int p = tid * KD_ITEMS + j;
+            unsigned low = 0u, r = 1u << t; /* pads: behind every sub-segment */
+            if (p < m) {
+                int ua, ub;
+                sub_of(p, t, ua, ub, r);
+                if (ub - ua <= LEAF) {
+                    low = (unsigned)(p - ua); /* keep the order of a final sub-segment */
+                } else {
+                    double ext[3];
+#pragma unroll
+                    for (int d = 0; d < 3; ++d)
+                        ext[d] = (double)nn_unordered(smax[r][d]) - (double)nn_unordered(smin[r][d]);
+                    int ax = 0; /* the first axis of the largest extent */
+                    if (ext[1] > ext[ax]) ax = 1;
+                    if (ext[2] > ext[ax]) ax = 2;
+                    const float* v = reinterpret_cast<const float*>(x + val[j]); /* second read: an L1 / L2 hit */
+                    low = nn_ordered(__ldg(v + ax));
+                }
+            }
+            key[j] = ((u64k)r << 32) | (u64k)low;
+        }
+        KdSort(sort_tmp).Sort(key, val, 0, 32 + t + 1);
+        __syncthreads();
+    }
+#pragma unroll
+    for (int j = 0; j < KD_ITEMS; ++j) {
+        const int p = tid * KD_ITEMS + j;
+        if (p < m) perm[a + p] = val[j];
+    }
+}
+
 /* one CTA per leaf: sorted copy (plain, padded) + blocked copy with header + bounding box + the two pseudo-particles.
  * Inside the leaf the members are put in the order negative weights first (a stable partition: which charges a leaf
  * holds is the k-d order's business, their order inside it enters no result), and perm_out records the final order.
@@ -292,27 +410,57 @@ __device__ __forceinline__ void nn_group_box(const float* __restrict__ leafbox, 
         }
 }
 
-/* one thread per super-leaf: union of its leaves' boxes, centres of charge from their fp64 moments (leaf order) */
-__global__ void nn_super_kernel(const float* __restrict__ leafbox, const double* __restrict__ leafmom, long long n_leaf,
-                                long long n_super, float* __restrict__ superbox, float4* __restrict__ superpseudo)
+/* one CTA of SUPER threads per super-leaf: union of its leaves' boxes (min / max: exact in any order), centres of
+ * charge from their fp64 moments, summed in leaf order by one thread per moment (from shared memory) */
+__global__ void __launch_bounds__(SUPER) nn_super_kernel(const float* __restrict__ leafbox,
+                                                         const double* __restrict__ leafmom, long long n_leaf,
+                                                         long long n_super, float* __restrict__ superbox,
+                                                         float4* __restrict__ superpseudo)
 {
-    const long long sidx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (sidx >= n_super) return;
+    __shared__ double mom[SUPER][9]; /* stride 9: the 8 summing threads read down the columns */
+    __shared__ float box[SUPER / 32][6];
+    __shared__ double tot[8];
+    const long long sidx = blockIdx.x;
+    const int t = threadIdx.x;
+    const long long l = sidx * SUPER + t;
     const float big = __int_as_float(0x7f800000);
     float b[6] = {big, big, big, -big, -big, -big};
-    double m[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    for (long long l = sidx * SUPER; l < (sidx + 1) * SUPER && l < n_leaf; ++l) {
-        for (int d = 0; d < 3; ++d) {
-            b[d] = fminf(b[d], leafbox[l * 6 + d]);
-            b[3 + d] = fmaxf(b[3 + d], leafbox[l * 6 + 3 + d]);
-        }
-        for (int k = 0; k < 8; ++k) m[k] += leafmom[l * 8 + k];
+    if (l < n_leaf) {
+#pragma unroll
+        for (int d = 0; d < 6; ++d) b[d] = leafbox[l * 6 + d];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mom[t][k] = leafmom[l * 8 + k];
     }
-    for (int d = 0; d < 6; ++d) superbox[sidx * 6 + d] = b[d];
-    for (int h = 0; h < 2; ++h) {
-        const double Q = m[4 * h];
-        superpseudo[sidx * 2 + h] = (Q != 0.0) ? make_float4((float)(m[4 * h + 1] / Q), (float)(m[4 * h + 2] / Q),
-                                                             (float)(m[4 * h + 3] / Q), (float)Q)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            b[d] = fminf(b[d], __shfl_xor_sync(0xffffffffu, b[d], o));
+            b[3 + d] = fmaxf(b[3 + d], __shfl_xor_sync(0xffffffffu, b[3 + d], o));
+        }
+    }
+    if ((t & 31) == 0) {
+#pragma unroll
+        for (int d = 0; d < 6; ++d) box[t >> 5][d] = b[d];
+    }
+    __syncthreads();
+    const int cnt = (int)min((long long)SUPER, n_leaf - sidx * SUPER);
+    if (t < 8) {
+        double m = 0.0;
+        for (int j = 0; j < cnt; ++j) m += mom[j][t];
+        tot[t] = m;
+    }
+    if (t >= 32 && t < 38) {
+        const int d = t - 32;
+        float v = box[0][d];
+        for (int w = 1; w < SUPER / 32; ++w) v = d < 3 ? fminf(v, box[w][d]) : fmaxf(v, box[w][d]);
+        superbox[sidx * 6 + d] = v;
+    }
+    __syncthreads();
+    if (t < 2) {
+        const double Q = tot[4 * t];
+        superpseudo[sidx * 2 + t] = (Q != 0.0) ? make_float4((float)(tot[4 * t + 1] / Q), (float)(tot[4 * t + 2] / Q),
+                                                             (float)(tot[4 * t + 3] / Q), (float)Q)
                                                : make_float4(NN_PAD_FAR, NN_PAD_FAR, NN_PAD_FAR, 0.f);
     }
 }
@@ -408,18 +556,37 @@ __global__ void __launch_bounds__(256) nn_lists_kernel(const float* __restrict__
     }
 }
 
-/* tile_ptr = exclusive prefix sum of cnt (n_group <= a few thousand: one thread), U = the total */
-__global__ void nn_scan_kernel(const long long* __restrict__ cnt, long long n_group, long long* __restrict__ tile_ptr,
-                               long long* __restrict__ U)
+/* tile_ptr = exclusive prefix sum of cnt, U = the total.  One CTA: every thread sums a run of consecutive tiles,
+ * the runs' totals are scanned across the block, then every thread writes its run (integers: exact in any order). */
+constexpr int SCAN_THREADS = 1024;
+__global__ void __launch_bounds__(SCAN_THREADS) nn_scan_kernel(const long long* __restrict__ cnt, long long n_group,
+                                                               long long* __restrict__ tile_ptr, long long* __restrict__ U)
 {
-    if (blockIdx.x || threadIdx.x) return;
+    __shared__ long long wtot[SCAN_THREADS / 32];
+    const int t = threadIdx.x, lane = t & 31, w = t >> 5;
+    const long long per = (n_group + SCAN_THREADS - 1) / SCAN_THREADS;
+    const long long g0 = min(n_group, (long long)t * per), g1 = min(n_group, g0 + per);
     long long s = 0;
-    for (long long g = 0; g < n_group; ++g) {
-        tile_ptr[g] = s;
-        s += cnt[g];
+    for (long long g = g0; g < g1; ++g) s += cnt[g];
+    long long inc = s; /* inclusive scan of the runs' totals: inside the warp, then across the warps */
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const long long v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
     }
-    tile_ptr[n_group] = s;
-    *U = s;
+    if (lane == 31) wtot[w] = inc;
+    __syncthreads();
+    long long before = 0;
+    for (int ww = 0; ww < w; ++ww) before += wtot[ww];
+    long long run = before + inc - s;
+    for (long long g = g0; g < g1; ++g) {
+        tile_ptr[g] = run;
+        run += cnt[g];
+    }
+    if (t == SCAN_THREADS - 1) {
+        tile_ptr[n_group] = before + inc;
+        *U = before + inc;
+    }
 }
 
 __global__ void nn_scatter_kernel(const float4* __restrict__ sorted_out, const int* __restrict__ perm, long long n,
@@ -533,7 +700,11 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     int cur = 0;
     unsigned* segmin = S.seg;
     unsigned* segmax = S.seg + n_leaf * 3;
-    for (int level = 0; level < levels; ++level) {
+    /* device-wide rounds while a segment can exceed KD_LOCAL_LEAVES leaves, then one launch for the rest */
+    int l0 = 0;
+    for (long long lv = n_leaf; lv > KD_LOCAL_LEAVES; lv = (lv + 1) / 2) ++l0;
+    if (l0 > levels) l0 = levels;
+    for (int level = 0; level < l0; ++level) {
         OBEM_CUDA(c, cudaMemsetAsync(segmin, 0xff, (size_t)n_leaf * 3 * sizeof(unsigned), st));
         OBEM_CUDA(c, cudaMemsetAsync(segmax, 0x00, (size_t)n_leaf * 3 * sizeof(unsigned), st));
         nn_segbox_kernel<<<gn, 256, 0, st>>>(c->d_chg, S.perm[cur], n, level, segmin, segmax);
@@ -545,13 +716,18 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
         cur ^= 1;
         c->launches += 3;
     }
+    if (l0 < levels) {
+        nn_kd_local_kernel<<<1u << l0, KD_THREADS, 0, st>>>(c->d_chg, S.perm[cur], n, l0, levels);
+        OBEM_CUDA(c, cudaGetLastError());
+        c->launches += 1;
+    }
     const int* perm = S.perm[cur];
     /* 2. leaves */
     nn_leaf_kernel<<<(unsigned)n_leaf, LEAF, 0, st>>>(c->d_chg, perm, n, S.sorted, S.pool, S.leafbox, S.pseudo,
                                                       S.leafmom, S.perm[cur ^ 1]);
     perm = S.perm[cur ^ 1]; /* the k-d order with the sign partition inside the leaves */
     OBEM_CUDA(c, cudaGetLastError());
-    nn_super_kernel<<<(unsigned)ceil_div(n_super, 64), 64, 0, st>>>(S.leafbox, S.leafmom, n_leaf, n_super, S.superbox,
+    nn_super_kernel<<<(unsigned)n_super, SUPER, 0, st>>>(S.leafbox, S.leafmom, n_leaf, n_super, S.superbox,
                                                                     S.superpseudo);
     OBEM_CUDA(c, cudaGetLastError());
     /* 3. + 4. per-tile lists and far blocks */
@@ -561,7 +737,7 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
     nn_lists_kernel<false><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, S.superbox, S.superpseudo, n_leaf,
                                                               n_super, far_cap, theta2, theta2s, S.cnt, nullptr, nullptr, nullptr);
     OBEM_CUDA(c, cudaGetLastError());
-    nn_scan_kernel<<<1, 32, 0, st>>>(S.cnt, n_group, S.tile_ptr, U_dev);
+    nn_scan_kernel<<<1, SCAN_THREADS, 0, st>>>(S.cnt, n_group, S.tile_ptr, U_dev);
     OBEM_CUDA(c, cudaGetLastError());
     nn_lists_kernel<true><<<(unsigned)n_group, 256, 0, st>>>(S.leafbox, S.pseudo, S.superbox, S.superpseudo, n_leaf,
                                                              n_super, far_cap, theta2, theta2s, S.cnt, S.tile_ptr, S.list, S.pool);
