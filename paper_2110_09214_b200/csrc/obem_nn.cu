@@ -177,20 +177,21 @@ __global__ void nn_key_kernel(const float4* __restrict__ x, const int* __restric
 
 /*
  * The last levels of the k-d order, one CTA per segment.  Once every segment holds at most KD_LOCAL_LEAVES leaves
- * (4096 charges) the remaining cuts touch nothing outside it: the CTA keeps the segment's 4096 (key, index) pairs in
+ * (8192 charges) the remaining cuts touch nothing outside it: the CTA keeps the segment's 8192 (key, index) pairs in
  * registers and runs the same rounds as the global loop -- boxes of the current sub-segments, axis = first of the
  * largest extents (fp64), STABLE sort by (sub-segment rank, ordered coordinate), cut at nn_split -- with a block-wide
  * radix sort instead of a device-wide one: the same order, bit for bit (a stable sort by the same keys), in one launch
  * instead of three launches + 5-6 radix passes per level.  CTA k takes the segment whose l0-bit path is k.
  */
-constexpr int KD_LOCAL_LEAVES = 16, KD_THREADS = 256, KD_ITEMS = KD_LOCAL_LEAVES * LEAF / KD_THREADS;
+constexpr int KD_LOCAL_LEAVES = 32, KD_THREADS = 512, KD_ITEMS = KD_LOCAL_LEAVES * LEAF / KD_THREADS;
 constexpr int KD_MAX_SUB = KD_LOCAL_LEAVES / 2; /* sub-segments that can still be cut in the last round */
 typedef cub::BlockRadixSort<u64k, KD_THREADS, KD_ITEMS, int, 6> KdSort; /* 6-bit digits: 6 passes over 33-36 key bits */
 
-__global__ void __launch_bounds__(KD_THREADS, 2) nn_kd_local_kernel(const float4* __restrict__ x, int* __restrict__ perm,
+__global__ void __launch_bounds__(KD_THREADS, 1) nn_kd_local_kernel(const float4* __restrict__ x, int* __restrict__ perm,
                                                                  long long n, int l0, int levels)
 {
-    __shared__ typename KdSort::TempStorage sort_tmp;
+    extern __shared__ __align__(16) unsigned char kd_dyn[]; /* sizeof(KdSort::TempStorage): above the static limit */
+    typename KdSort::TempStorage& sort_tmp = *reinterpret_cast<typename KdSort::TempStorage*>(kd_dyn);
     __shared__ unsigned smin[2 * KD_MAX_SUB][3], smax[2 * KD_MAX_SUB][3];
     long long a = 0, b = n;
     for (int t = 0; t < l0; ++t) {
@@ -717,7 +718,9 @@ int obem_eval_at_charges_nn(obem_ctx* c, float* d_out, unsigned flags, void* cud
         c->launches += 3;
     }
     if (l0 < levels) {
-        nn_kd_local_kernel<<<1u << l0, KD_THREADS, 0, st>>>(c->d_chg, S.perm[cur], n, l0, levels);
+        OBEM_CUDA(c, cudaFuncSetAttribute(nn_kd_local_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)sizeof(KdSort::TempStorage)));
+        nn_kd_local_kernel<<<1u << l0, KD_THREADS, sizeof(KdSort::TempStorage), st>>>(c->d_chg, S.perm[cur], n, l0, levels);
         OBEM_CUDA(c, cudaGetLastError());
         c->launches += 1;
     }
