@@ -138,16 +138,19 @@ def test_config4_charges_full_size_sampled_groups(torch_cuda, api, ctx, nn, ref)
     assert units * 2048 * 256 < 0.02 * wl.n_charges * (wl.n_charges - 1.0)
 
 
-@pytest.mark.parametrize("n", [1, 2, 255, 256, 257, 2047, 2049, 4097])
+# 8191 .. 16641: around 32 / 33 / 64 / 65 leaves, where the k-d order changes from device-wide rounds to the one-launch
+# rounds of nn_kd_local_kernel (segments of at most 32 leaves); below that everything is local
+@pytest.mark.parametrize("n", [1, 2, 255, 256, 257, 2047, 2049, 4097, 8191, 8192, 8193, 8449, 16385, 16641])
 def test_small_and_ragged_sizes(torch_cuda, ctx, nn, ref, n):
     rng = np.random.default_rng([61, 7, n])
     x = _cloud(rng, n)
-    exp, _ = nn.nn_field(x, 0.1 * UM, 2.0, ref=ref)
+    exp, tree = nn.nn_field(x, 0.1 * UM, 2.0, ref=ref)
     got = _gpu_nn(torch_cuda, ctx, x, 0.1 * UM, 2.0)
     if n == 1:
         assert np.all(got == 0)
     else:
         assert_parity(got, exp, "nn n=%d" % n)
+    assert ctx.nn_last_units() == nn.units(tree, 2.0, n)     # the same leaves, the same near / far decisions
 
 
 def test_degenerate_positions(torch_cuda, ctx, nn, ref):
