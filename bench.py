@@ -708,7 +708,7 @@ def bench_next1(torch, api, ctx, wl, timed, dev, t_panels):
     t_ramo = timed(lambda: ctx.ramo_current(pts, vel, out4), reps=5)
     peak_hbm, src_hbm = hbm_peak_gbs()
     ramo_bytes = n * (16 * 4 + 32)
-    res["ramo_current_4"] = {"s": t_ramo, "bound": "hbm (two launches: latency-bound at this size)",
+    res["ramo_current_4"] = {"s": t_ramo, "bound": "hbm (two launches)",
                              "algorithmic_bytes": ramo_bytes, "achieved": ramo_bytes / t_ramo / 1e9, "peak": peak_hbm,
                              "unit": "GB/s", "frac": ramo_bytes / t_ramo / 1e9 / peak_hbm, "peak_source": src_hbm}
     del sig4, out4, pts, vel

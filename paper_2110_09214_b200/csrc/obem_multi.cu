@@ -300,8 +300,8 @@ __global__ void __launch_bounds__(M_THREADS, 1) panels_multi_kernel(const MultiP
  * The Shockley-Ramo signal sum, Eq (3.13): i_k = sum_p q_p v_p . E_w^(k)(r_p), separately for the
  * particles with q < 0 and with q > 0 ("the signals created by each type are generated separately").
  * ew [K][n] is what obem_eval_panels_multi writes for K weighting-field density vectors at the charges.  fp32 inputs,
- * every term and every sum in fp64, fixed summation order (strided per thread, tree per block, blocks in order): the
- * result is deterministic.  Bound: HBM (16 B of E_w per particle and electrode; q and v come from L2 after the first
+ * every term and every sum in fp64, fixed summation order (strided per thread, tree per block; the blocks' partials
+ * the same way in a second launch): the result is deterministic.  Bound: HBM (16 B of E_w per particle and electrode; q and v come from L2 after the first
  * electrode).  Grid: (blocks, K).
  */
 constexpr int R_THREADS = 256;
@@ -313,6 +313,7 @@ __global__ void __launch_bounds__(R_THREADS) ramo_partial_kernel(const float4* _
     const int tid = threadIdx.x, k = blockIdx.y;
     const long long i0 = (long long)blockIdx.x * chunk, i1 = (i0 + chunk < n) ? i0 + chunk : n;
     double neg = 0.0, pos = 0.0;
+#pragma unroll 4
     for (long long i = i0 + tid; i < i1; i += R_THREADS) {
         const float q = xyzq[i].w;
         const float4 v = vel[i], e = ew[(long long)k * n + i];
@@ -331,13 +332,24 @@ __global__ void __launch_bounds__(R_THREADS) ramo_partial_kernel(const float4* _
         part[((size_t)k * gridDim.x + blockIdx.x) * 2 + 1] = red[1][0];
     }
 }
-__global__ void ramo_final_kernel(const double* __restrict__ part, int blocks, int K, double* __restrict__ out)
+/* one CTA per electrode: thread t sums the partials t, t + 256, ... in ascending order, then the same fixed tree */
+__global__ void __launch_bounds__(R_THREADS) ramo_final_kernel(const double* __restrict__ part, int blocks, int K,
+                                                               double* __restrict__ out)
 {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= K) return;
+    __shared__ double red[2][R_THREADS];
+    const int tid = threadIdx.x, k = blockIdx.x;
     double neg = 0.0, pos = 0.0;
-    for (int b = 0; b < blocks; ++b) neg += part[((size_t)k * blocks + b) * 2], pos += part[((size_t)k * blocks + b) * 2 + 1];
-    out[2 * k] = neg, out[2 * k + 1] = pos;
+    for (int b = tid; b < blocks; b += R_THREADS) {
+        neg += part[((size_t)k * blocks + b) * 2];
+        pos += part[((size_t)k * blocks + b) * 2 + 1];
+    }
+    red[0][tid] = neg, red[1][tid] = pos;
+    __syncthreads();
+    for (int h = R_THREADS / 2; h > 0; h >>= 1) {
+        if (tid < h) red[0][tid] += red[0][tid + h], red[1][tid] += red[1][tid + h];
+        __syncthreads();
+    }
+    if (tid == 0) out[2 * k] = red[0][0], out[2 * k + 1] = red[1][0];
 }
 
 template <int KS>
@@ -471,7 +483,7 @@ extern "C" int obem_ramo_current(obem_ctx* c, const float* d_xyzq, const float* 
     ramo_partial_kernel<<<dim3((unsigned)blocks, (unsigned)n_electrodes), R_THREADS, 0, st>>>(
         (const float4*)d_xyzq, (const float4*)d_vel, (const float4*)d_ew, n, chunk, c->d_ramo);
     OBEM_CUDA(c, cudaGetLastError());
-    ramo_final_kernel<<<(unsigned)ceil_div(n_electrodes, 64), 64, 0, st>>>(c->d_ramo, (int)blocks, n_electrodes, d_out);
+    ramo_final_kernel<<<(unsigned)n_electrodes, R_THREADS, 0, st>>>(c->d_ramo, (int)blocks, n_electrodes, d_out);
     OBEM_CUDA(c, cudaGetLastError());
     c->launches += 2;
     return OBEM_OK;
