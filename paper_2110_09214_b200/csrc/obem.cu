@@ -271,6 +271,9 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
 #ifndef OBEM_KNOBS_E
 #define OBEM_KNOBS_E 6201
 #endif
+#ifndef OBEM_KNOBS_L
+#define OBEM_KNOBS_L 6301 /* the NN list launch (LIST instantiation): its own sweep, 48 + 37 variants on config 3 */
+#endif
 #ifndef OBEM_KNOBS_T
 #define OBEM_KNOBS_T 3001
 #endif
@@ -286,6 +289,8 @@ struct Knobs {
 };
 constexpr Knobs knobs_of(int code) { return Knobs{code / 1000, (code / 100) % 10, (code / 10) % 10, code % 10}; }
 constexpr Knobs KNOBS_PHI = knobs_of(OBEM_KNOBS_PHI), KNOBS_E = knobs_of(OBEM_KNOBS_E), KNOBS_T = knobs_of(OBEM_KNOBS_T);
+constexpr Knobs KNOBS_L = knobs_of(OBEM_KNOBS_L);
+static_assert(KNOBS_L.vf == KNOBS_PHI.vf, "VF changes the rounding of r2: one value for all");
 constexpr Knobs PKNOBS_PHI = knobs_of(OBEM_PKNOBS_PHI), PKNOBS_E = knobs_of(OBEM_PKNOBS_E);
 static_assert(KNOBS_PHI.vf == KNOBS_E.vf && KNOBS_PHI.vf == KNOBS_T.vf, "VF changes the rounding of r2: one value for all");
 
@@ -313,14 +318,14 @@ __device__ __forceinline__ void uni_front(u64& dx, u64& dy, u64& dz, u64& u, flo
  * weight is applied once per block (by the caller) and the body is 12 packed instructions: phi += u, u^2, u^3,
  * E += u^3 d.
  */
-template <bool TRACK, bool PHI, int NS, int NPAIR>
+template <bool TRACK, bool PHI, int NS, int NPAIR, bool LISTK = false>
 __device__ __forceinline__ void block_loop_uniform(const float4* __restrict__ s, const float eps2,
                                                    const u64 (&X)[NPAIR], const u64 (&Y)[NPAIR],
                                                    const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR], u64 (&aY)[NPAIR],
                                                    u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[2 * NPAIR],
                                                    const int jb = 0, const int je = NS)
 {
-    constexpr Knobs KN = TRACK ? KNOBS_T : (PHI ? KNOBS_PHI : KNOBS_E);
+    constexpr Knobs KN = TRACK ? KNOBS_T : (PHI ? (LISTK ? KNOBS_L : KNOBS_PHI) : KNOBS_E);
     constexpr int DEPTH = KN.d;
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR;
@@ -773,8 +778,8 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
                 u64 bX[NPAIR], bY[NPAIR], bZ[NPAIR], bP[NPAIR];
 #pragma unroll
                 for (int p = 0; p < NPAIR; ++p) bX[p] = bY[p] = bZ[p] = bP[p] = 0ull;
-                block_loop_uniform<false, PHI, SB, NPAIR>(sblk, eps2, X, Y, Z, bX, bY, bZ, bP, bm, 0, n4);
-                block_loop_uniform<false, PHI, SB, NPAIR>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, bm, n4 + 4 < SB ? n4 + 4 : SB, SB);
+                block_loop_uniform<false, PHI, SB, NPAIR, true>(sblk, eps2, X, Y, Z, bX, bY, bZ, bP, bm, 0, n4);
+                block_loop_uniform<false, PHI, SB, NPAIR, true>(sblk, eps2, X, Y, Z, aX, aY, aZ, aP, bm, n4 + 4 < SB ? n4 + 4 : SB, SB);
                 const u64 w2 = pk(wmag, wmag);
 #pragma unroll
                 for (int p = 0; p < NPAIR; ++p) {
@@ -787,7 +792,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             } else if (blkw == blkw) {
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)
-                    block_loop_uniform<TRACK, PHI, NSP, NPAIR>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
+                    block_loop_uniform<TRACK, PHI, NSP, NPAIR, LIST>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
                 phi_join();
                 const u64 w2 = pk(blkw, blkw);
 #pragma unroll
