@@ -210,15 +210,24 @@ __device__ __forceinline__ float min3_nonneg(float a, float b, float c)
 {
     return __int_as_float(__vimin3_s32(__float_as_int(a), __float_as_int(b), __float_as_int(c)));
 }
+/* statement order of the weighted loop inside the NN list launch (its far blocks): three decimal digits + 0, as the
+ * knobs of the uniform loop below (D, VE, VP); 0 = the common order.  8100: best of 72 + 42 variants on config 3. */
+#ifndef OBEM_KNOBS_LB
+#define OBEM_KNOBS_LB 8100
+#endif
 /* One block of SB point sources against the thread's TPT targets (KIND_POINTS).  Unguarded: see the
  * "speculative zero-distance handling" note at obem_repair_kernel. */
-template <bool TRACK, bool PHI, int NS, int NPAIR>
+template <bool TRACK, bool PHI, int NS, int NPAIR, bool LISTK = false>
 __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const float eps2, const u64 (&X)[NPAIR],
                                            const u64 (&Y)[NPAIR], const u64 (&Z)[NPAIR], u64 (&aX)[NPAIR],
                                            u64 (&aY)[NPAIR], u64 (&aZ)[NPAIR], u64 (&aP)[NPAIR], float (&bm)[2 * NPAIR])
 {
     const u64 e2 = pk(eps2, eps2);
     constexpr int K = UNR * NPAIR; /* work items (source, target pair) per trip */
+    /* statement order: the common one, or the NN list launch's own (OBEM_KNOBS_LB, see the knobs below) */
+    constexpr bool OWN = LISTK && OBEM_KNOBS_LB != 0;
+    constexpr int DEPTH_B = OWN ? OBEM_KNOBS_LB / 1000 : DEPTH, VE = OWN ? (OBEM_KNOBS_LB / 100) % 10 : 0,
+                  VP = OWN ? (OBEM_KNOBS_LB / 10) % 10 : 0;
 #pragma unroll 1
     for (int j0 = 0; j0 < NS; j0 += UNR) {
         float4 q[UNR];
@@ -229,7 +238,7 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
         /* software pipeline over the K items of the trip: item k's distance + rsqrt are issued DEPTH
          * items before its accumulation, so the MUFU latency is covered by independent FFMA2 work */
 #pragma unroll
-        for (int k = 0; k < K + DEPTH; ++k) {
+        for (int k = 0; k < K + DEPTH_B; ++k) {
             if (k < K) {
                 const int j = k / NPAIR, p = k % NPAIR;
                 if (TRACK) { /* as in block_loop_uniform: the block is of one sign (header .y), decided after the block */
@@ -243,16 +252,27 @@ __device__ __forceinline__ void block_loop(const float4* __restrict__ s, const f
                     item_front<false>(dX[k], dY[k], dZ[k], U[k], X[p], Y[p], Z[p], q[j].x, q[j].y, q[j].z, e2);
                 }
             }
-            if (k >= DEPTH) {
-                const int kk = k - DEPTH, j = kk / NPAIR, p = kk % NPAIR;
+            if (k >= DEPTH_B) {
+                const int kk = k - DEPTH_B, j = kk / NPAIR, p = kk % NPAIR;
                 /* as item_back, with phi summed as a tree over the 4 sources of the trip (see block_loop_uniform) */
                 W[kk] = mul2(U[kk], pk(q[j].w, q[j].w));
-                if (PHI && j == 1) T[p] = add2(W[kk - NPAIR], W[kk]);
-                if (PHI && j == 3) aP[p] = add2(aP[p], add2(T[p], add2(W[kk - NPAIR], W[kk])));
+                if (VP == 0) {
+                    if (PHI && j == 1) T[p] = add2(W[kk - NPAIR], W[kk]);
+                    if (PHI && j == 3) aP[p] = add2(aP[p], add2(T[p], add2(W[kk - NPAIR], W[kk])));
+                }
                 const u64 sE = mul2(W[kk], mul2(U[kk], U[kk]));
-                aX[p] = fma2(sE, dX[kk], aX[p]);
-                aY[p] = fma2(sE, dY[kk], aY[p]);
-                aZ[p] = fma2(sE, dZ[kk], aZ[p]);
+                if (VP == 1) {
+                    if (PHI && j == 1) T[p] = add2(W[kk - NPAIR], W[kk]);
+                    if (PHI && j == 3) aP[p] = add2(aP[p], add2(T[p], add2(W[kk - NPAIR], W[kk])));
+                }
+                if (VE == 0) { aX[p] = fma2(sE, dX[kk], aX[p]); aY[p] = fma2(sE, dY[kk], aY[p]); aZ[p] = fma2(sE, dZ[kk], aZ[p]); }
+                if (VE == 1) { aZ[p] = fma2(sE, dZ[kk], aZ[p]); aY[p] = fma2(sE, dY[kk], aY[p]); aX[p] = fma2(sE, dX[kk], aX[p]); }
+                if (VE == 2) { aY[p] = fma2(sE, dY[kk], aY[p]); aX[p] = fma2(sE, dX[kk], aX[p]); aZ[p] = fma2(sE, dZ[kk], aZ[p]); }
+                if (VE == 3) { aX[p] = fma2(sE, dX[kk], aX[p]); aZ[p] = fma2(sE, dZ[kk], aZ[p]); aY[p] = fma2(sE, dY[kk], aY[p]); }
+                if (VP == 2) {
+                    if (PHI && j == 1) T[p] = add2(W[kk - NPAIR], W[kk]);
+                    if (PHI && j == 3) aP[p] = add2(aP[p], add2(T[p], add2(W[kk - NPAIR], W[kk])));
+                }
             }
         }
     }
@@ -788,7 +808,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
                     aZ[p] = mul2(sub2(aZ[p], bZ[p]), w2);
                     if (PHI) aP[p] = mul2(sub2(aP[p], bP[p]), w2);
                 }
-                if (n4 < SB) block_loop<false, PHI, 4, NPAIR>(sblk + n4, eps2, X, Y, Z, aX, aY, aZ, aP, bm);
+                if (n4 < SB) block_loop<false, PHI, 4, NPAIR, true>(sblk + n4, eps2, X, Y, Z, aX, aY, aZ, aP, bm);
             } else if (blkw == blkw) {
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)
@@ -806,7 +826,7 @@ __global__ void __launch_bounds__(THREADS, CTAS_PER_SM) obem_eval_kernel(const E
             } else {
 #pragma unroll
                 for (int h = 0; h < PARTS; ++h)
-                    block_loop<TRACK, PHI, NSP, NPAIR>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
+                    block_loop<TRACK, PHI, NSP, NPAIR, LIST>(sblk + h * NSP, eps2, X, Y, Z, aX, aY, aZ, h == 0 ? aP : aQ[h > 0 ? h - 1 : 0], bm);
                 phi_join();
                 elig = (blks > 0.f) ? negmask : ((blks < 0.f) ? posmask : 0u);
             }
