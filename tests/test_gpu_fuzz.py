@@ -4,6 +4,8 @@ evaluation at the charges / at a slice of them / at free points, symmetry planes
 exactly representable), exact near-field integrals.  Catches interactions between features that the per-feature tests
 do not combine.  `pytest -m gpu`.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -77,7 +79,8 @@ def _images(xyzq, verts, sigma, planes):
     return np.concatenate(xs), np.concatenate(vs), np.concatenate(ss)
 
 
-@pytest.mark.parametrize("seed", range(64))
+# OBEM_FUZZ_SEEDS=N runs N seeds instead of 64
+@pytest.mark.parametrize("seed", range(int(os.environ.get("OBEM_FUZZ_SEEDS", "64"))))
 def test_random_combination(torch_cuda, api, ref, seed):
     k = _case(seed)
     rng, n = k["rng"], k["n"]
